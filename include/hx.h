@@ -1,0 +1,108 @@
+/*
+ * hx.h -- C ABI of the B200-native fp64 Godunov finite-volume hydro step
+ * (hot path of HERACLES++, arxiv 2503.04428; Sect. 2-3).
+ *
+ * One handle = one logically Cartesian block on one GPU (Sect. 3.1.1).  The library
+ * owns every device allocation: the double-buffered conserved state, stored as structure-of-arrays
+ * fp64 [nvar][n2+4][n1+4][pitch0] with two ghost layers per face in active directions, and the 1-D
+ * geometry tables.  Caller buffers are only read or written during hx_set_state / hx_get_state;
+ * nothing is retained.  All calls are host functions; kernels run on the handle's stream.
+ *
+ * Caller state buffers are interior-only structure-of-arrays [nvar][n2][n1][n0], direction 0
+ * fastest, nvar = 2 + ndim + n_scalars, field order
+ *     HX_CONSERVED: rho, m_0..m_{ndim-1}, E, rho*f_1..rho*f_ns          (Eq. 1a-1d)
+ *     HX_PRIMITIVE: rho, u_0..u_{ndim-1}, P, f_1..f_ns                  (Eq. 5)
+ * Directions are (x,y,z) or, with HX_SPHERICAL, (r,theta,phi) (L145).
+ *
+ * Errors: every function returns HX_OK or a negative code; nothing throws, exits or prints.
+ * hx_last_error() gives a message for the last failing call on that handle.  There is no CPU
+ * fallback: without a CUDA device hx_create fails with HX_ERR_CUDA.
+ */
+#ifndef HX_H
+#define HX_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hx_handle hx_handle;
+
+enum { HX_OK = 0, HX_ERR_INVALID_ARG = -1, HX_ERR_ALLOC = -2, HX_ERR_CUDA = -3,
+       HX_ERR_NONPHYSICAL = -4 /* rho<=0, P<=0 or non-finite seen */, HX_ERR_UNSUPPORTED = -5 };
+enum { HX_CARTESIAN = 0, HX_SPHERICAL = 1 };
+/* Boundary conditions (periodic, null gradient, reflective).  HX_BC_WEDGE is the
+ * reflective condition on the angular faces of a spherical wedge (L424). */
+enum { HX_BC_PERIODIC = 0, HX_BC_TRANSMISSIVE = 1, HX_BC_REFLECTING = 2, HX_BC_WEDGE = 3 };
+enum { HX_EOS_IDEAL = 0 };                              /* Eq. 5 */
+enum { HX_RIEMANN_HLL = 0, HX_RIEMANN_HLLC = 1 };       /* L201 */
+/* Slope limiters (L189) + first order (HX_LIM_NONE) + monotonised central (BASELINE.json configs) */
+enum { HX_LIM_NONE = 0, HX_LIM_MINMOD = 1, HX_LIM_VANLEER = 2, HX_LIM_VANALBADA = 3, HX_LIM_MC = 4 };
+enum { HX_GRAV_NONE = 0, HX_GRAV_UNIFORM = 1 /* Eq. 2 */, HX_GRAV_POINT_MASS = 2 /* Eq. 3 */ };
+enum { HX_SPACING_UNIFORM = 0, HX_SPACING_LOG = 1, HX_SPACING_CUSTOM = 2 };   /* L149 */
+enum { HX_HOST = 0, HX_DEVICE = 1 };
+enum { HX_CONSERVED = 0, HX_PRIMITIVE = 1 };
+/* Step kernel selection (hx_set_option(HX_OPT_KERNEL, ..)): AUTO picks the fused tile kernel where
+ * it applies and the generic one elsewhere; the other two force one path (tests, profiling). */
+enum { HX_OPT_KERNEL = 0, HX_OPT_TIMING = 1 /* 0/1: bracket each step-kernel launch with CUDA events */ };
+enum { HX_KERNEL_AUTO = 0, HX_KERNEL_GENERIC = 1, HX_KERNEL_TILED = 2 };
+
+#define HX_MAX_NVAR 16
+
+typedef struct {
+  int ndim;               /* 1, 2 or 3; active directions are 0..ndim-1                              */
+  int coords;             /* HX_CARTESIAN or HX_SPHERICAL                                            */
+  int n[3];               /* interior cells; inactive directions must be 1; active ones >= 2         */
+  double lo[3], hi[3];    /* extents.  Inactive directions: Cartesian width hi-lo (1 if hi<=lo);     */
+                          /* spherical theta defaults to [0,pi] and phi to [0,2pi] if hi<=lo         */
+  int spacing[3];         /* per direction: uniform, logarithmic (lo>0) or custom                    */
+  const double* faces[3]; /* HX_SPACING_CUSTOM: n[d]+1 strictly increasing HOST face coordinates,    */
+                          /* copied during hx_create                                                 */
+  int bc_lo[3], bc_hi[3]; /* periodic must be set on both sides of a direction                       */
+  int eos;                /* HX_EOS_IDEAL                                                            */
+  double gamma;           /* adiabatic index > 1                                                     */
+  int riemann, limiter, n_scalars;
+  int gravity;            /* HX_GRAV_*; point mass needs HX_SPHERICAL                                */
+  double g[3];            /* uniform: acceleration vector (force = +rho*g, R12)            */
+  double GM;              /* point mass: g = -GM/r_c^2 e_r                                           */
+} hx_config;
+
+/* Validate cfg, allocate the padded double-buffered state and the geometry tables on the current
+ * CUDA device.  *out is NULL on failure. */
+int hx_create(const hx_config* cfg, hx_handle** out);
+/* Free everything the handle owns.  NULL is accepted. */
+int hx_destroy(hx_handle* h);
+/* Use the given cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) for all later work.
+ * NULL = the legacy default stream.  The caller keeps ownership of the stream. */
+int hx_set_stream(hx_handle* h, void* cuda_stream);
+int hx_set_option(hx_handle* h, int option, int value);
+/* Copy the caller's interior state in (mem_space = HX_HOST or HX_DEVICE pointer; form = conserved
+ * or primitive, converted through the EOS).  Returns after the copy is enqueued (device pointer)
+ * or finished (host pointer). */
+int hx_set_state(hx_handle* h, const double* data, int mem_space, int form);
+/* Copy the interior state out; synchronises the stream.  Returns HX_ERR_NONPHYSICAL (after
+ * copying) if a kernel flagged a non-physical state since the last hx_set_state. */
+int hx_get_state(hx_handle* h, double* data, int mem_space, int form);
+/* A7: dt = cfl / max over interior cells of sum_d (|u_d|+c_s)/l_d (R2).  Uses the rate
+ * the last hx_step folded into its update when available, else runs the reduction kernel.
+ * Synchronises the stream (one 16-byte device-to-host copy). */
+int hx_compute_dt(hx_handle* h, double cfl, double* dt_out);
+/* A0-A6 (+A7 fused): ghost fill, then one unsplit MUSCL-Hancock / Godunov update of every interior
+ * cell by dt (Eq. 17-19, sources Eq. 13-16, gravity Eq. 2-3).  Asynchronous on the stream; device
+ * side errors surface at the next hx_compute_dt / hx_get_state. */
+int hx_step(hx_handle* h, double dt);
+/* Number of stored fields, 2 + ndim + n_scalars. */
+int hx_nvar(const hx_handle* h);
+/* Kernels launched by this handle so far (for bench.py's gpu_launches). */
+long long hx_launch_count(const hx_handle* h);
+/* With HX_OPT_TIMING on: device time (ms) spent in the step kernel alone, summed over the launches
+ * measured so far, and their number.  Read after a synchronising call (hx_compute_dt / hx_get_state);
+ * a launch whose events were not yet collected when the next step started is not counted. */
+int hx_kernel_time(hx_handle* h, double* total_ms, long long* launches);
+/* Name of the step kernel the last hx_step used ("generic", "tiled3d", ..). */
+const char* hx_step_kernel_name(const hx_handle* h);
+const char* hx_last_error(const hx_handle* h);
+const char* hx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

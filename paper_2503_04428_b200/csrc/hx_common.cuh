@@ -1,0 +1,197 @@
+// hx_common.cuh -- shared declarations of the CUDA path (layout, geometry tables, pointwise physics).
+// Hand-written for sm_100a.  Shares nothing with oracle/.
+//
+// Pointwise physics follows PAPER.md: Eq. 1 + Eq. 5 (cons <-> prim, ideal gas), Eq. 17 (limited
+// slopes), Eq. 18 (Hancock predictor), Eq. 19 with HLL / HLLC (L197-L201), readings R1-R25 of DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "../../include/hx.h"
+
+namespace hx {
+
+constexpr int NG = 2;                 // ghost layers per face in active directions
+constexpr int NVMAX = HX_MAX_NVAR;
+
+// Padded structure-of-arrays layout [nvar][np2][np1][pitch0]; offsets in doubles.
+struct Layout {
+  int ndim, nvar;
+  int n[3];    // interior cells
+  int ng[3];   // NG for active directions, 0 otherwise
+  int np[3];   // n + 2 ng
+  int lead;    // doubles of padding in front of each x row (alignment of the first interior cell)
+  long long sy, sz, sv;   // strides of j, k, variable
+  __host__ __device__ long long off(int pi, int pj, int pk) const { return (long long)pk * sz + (long long)pj * sy + pi + lead; }
+};
+
+// 1-D geometry tables, all indexed by the padded cell index of their axis.
+// Face-area / volume ratios are products of per-axis factors:
+//   dS_{d,-}/dV = cf[d][0][0][pi] * cf[d][0][1][pj] * cf[d][0][2][pk],   dS_{d,+}/dV likewise with cf[d][1].
+// CFL lengths: 1/l_d = lf[d][0][pi] * lf[d][1][pj] * lf[d][2][pk].
+struct Tables {
+  const double* cf[3][2][3];
+  const double* lf[3][3];
+  const double* idx[3];   // idx[d][p] = 1 / (xc[p] - xc[p-1])   (p >= 1)
+  const double* hw[3];    // half cell width
+  const double* grav[3];  // acceleration component along d seen by cell p (mirrored behind reflecting faces, R25)
+  // spherical source factors
+  const double* gr;   // by i: (dS^r+ - dS^r-)/(2 dV)
+  const double* Ar;   // by i: (r+ - r-)(dS^r+ + dS^r-)/((r+ + r-) dV)
+  const double* rr;   // by i: (r+ - r-)/(r+ + r-)
+  const double* cr;   // by i: ((r+^2 - r-^2)/2) / ((r+^3 - r-^3)/3)
+  const double* gt;   // by j: (sin th+ - sin th-)/(cos th- - cos th+)
+  const double* At;   // by j: st * (sin th+ + sin th-)/(cos th- - cos th+)
+  const double* st;   // by j: (sin th+ - sin th-)/(sin th+ + sin th-)
+};
+
+struct Phys {
+  double gamma, gm1, igm1;
+  int limiter, riemann, gravity, spherical;
+};
+
+struct StepArgs {
+  Layout L;
+  Tables T;
+  Phys P;
+  const double* __restrict__ Uin;
+  double* __restrict__ Uout;
+  double dt;
+  unsigned long long* rate_bits;   // max over cells of the CFL rate of the NEW state (bit pattern of a double >= 0)
+  int* status;                     // bit 0: non-physical state seen
+};
+
+// ---------------------------------------------------------------------------------------------
+// Limiters (Eq. 17; R3-R5).  a = backward gradient, b = forward gradient.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double limited_slope(int lim, double a, double b) {
+  if (lim == HX_LIM_NONE) return 0.0;
+  const double ab = a * b;
+  if (!(ab > 0.0)) return 0.0;
+  const double fa = fabs(a), fb = fabs(b);
+  double s;
+  switch (lim) {
+    case HX_LIM_MINMOD: s = fmin(fa, fb); break;
+    case HX_LIM_VANLEER: s = 2.0 * fa * fb / (fa + fb); break;
+    case HX_LIM_VANALBADA: s = fa * fb * (fa + fb) / (fa * fa + fb * fb); break;
+    default: s = fmin(fmin(2.0 * fa, 2.0 * fb), 0.5 * (fa + fb)); break;   // MC
+  }
+  return copysign(s, a);
+}
+
+// ---------------------------------------------------------------------------------------------
+// cons <-> prim (Eq. 1, Eq. 5).  Field order: rho, m_d / u_d (ND of them), E / P, scalars.
+// ---------------------------------------------------------------------------------------------
+template <int ND>
+__device__ __forceinline__ void cons_to_prim(const Phys& P, int nv, const double* U, double* W) {
+  const double rho = U[0];
+  const double ir = 1.0 / rho;
+  W[0] = rho;
+  double u2 = 0.0;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    W[1 + d] = U[1 + d] * ir;
+    u2 += W[1 + d] * W[1 + d];
+  }
+  W[1 + ND] = P.gm1 * (U[1 + ND] - 0.5 * rho * u2);
+  for (int s = 2 + ND; s < nv; ++s) W[s] = U[s] * ir;
+}
+
+template <int ND>
+__device__ __forceinline__ void prim_to_cons(const Phys& P, int nv, const double* W, double* U) {
+  const double rho = W[0];
+  U[0] = rho;
+  double u2 = 0.0;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    U[1 + d] = rho * W[1 + d];
+    u2 += W[1 + d] * W[1 + d];
+  }
+  U[1 + ND] = W[1 + ND] * P.igm1 + 0.5 * rho * u2;
+  for (int s = 2 + ND; s < nv; ++s) U[s] = rho * W[s];
+}
+
+// Analytic flux along dir from primitives W and the matching conserved U (Eq. 1).
+template <int ND>
+__device__ __forceinline__ void flux_along(int nv, int dir, const double* W, const double* U, double* F) {
+  const double un = W[1 + dir];
+  const double p = W[1 + ND];
+  F[0] = U[0] * un;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) F[1 + d] = U[1 + d] * un + (d == dir ? p : 0.0);
+  F[1 + ND] = (U[1 + ND] + p) * un;
+  for (int s = 2 + ND; s < nv; ++s) F[s] = U[s] * un;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Riemann flux across a face normal to dir between conserved states UL | UR (L197-L201; Toro 2009
+// ch. 10; Davis wave speeds R14; ties R15).
+// ---------------------------------------------------------------------------------------------
+template <int ND, int NVA>
+__device__ __forceinline__ void riemann_flux(const Phys& P, int nv, int dir, const double* UL, const double* UR, double* F) {
+  double WL[NVA], WR[NVA], FL[NVA], FR[NVA];
+  cons_to_prim<ND>(P, nv, UL, WL);
+  cons_to_prim<ND>(P, nv, UR, WR);
+  flux_along<ND>(nv, dir, WL, UL, FL);
+  flux_along<ND>(nv, dir, WR, UR, FR);
+  const double rL = WL[0], rR = WR[0], uL = WL[1 + dir], uR = WR[1 + dir], pL = WL[1 + ND], pR = WR[1 + ND];
+  const double cL = sqrt(P.gamma * pL / rL), cR = sqrt(P.gamma * pR / rR);
+  const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
+  if (P.riemann == HX_RIEMANN_HLL) {
+    if (SL >= 0.0) {
+      for (int v = 0; v < nv; ++v) F[v] = FL[v];
+    } else if (SR <= 0.0) {
+      for (int v = 0; v < nv; ++v) F[v] = FR[v];
+    } else {
+      const double iw = 1.0 / (SR - SL);
+      for (int v = 0; v < nv; ++v) F[v] = (SR * FL[v] - SL * FR[v] + SL * SR * (UR[v] - UL[v])) * iw;
+    }
+    return;
+  }
+  const double mL = rL * (SL - uL), mR = rR * (SR - uR);
+  const double Ss = (pR - pL + uL * mL - uR * mR) / (mL - mR);
+  const bool left = (Ss >= 0.0);
+  if (SL >= 0.0) {
+    for (int v = 0; v < nv; ++v) F[v] = FL[v];
+  } else if (!left && SR <= 0.0) {
+    for (int v = 0; v < nv; ++v) F[v] = FR[v];
+  } else {
+    const double* UK = left ? UL : UR;
+    const double* WK = left ? WL : WR;
+    const double* FK = left ? FL : FR;
+    const double SK = left ? SL : SR, mK = left ? mL : mR, uK = left ? uL : uR, pK = left ? pL : pR, rK = left ? rL : rR;
+    const double fac = mK / (SK - Ss);
+    F[0] = FK[0] + SK * (fac - UK[0]);
+#pragma unroll
+    for (int d = 0; d < ND; ++d) F[1 + d] = FK[1 + d] + SK * (fac * (d == dir ? Ss : WK[1 + d]) - UK[1 + d]);
+    F[1 + ND] = FK[1 + ND] + SK * (fac * (UK[1 + ND] / rK + (Ss - uK) * (Ss + pK / mK)) - UK[1 + ND]);
+    for (int s = 2 + ND; s < nv; ++s) F[s] = FK[s] + SK * (fac * WK[s] - UK[s]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Reductions
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Block-wide max of a non-negative double, one atomicMax per block on its bit pattern (positive
+// IEEE doubles order like unsigned integers).  All threads of the block must call it.
+__device__ __forceinline__ void block_rate_max(double rate, unsigned long long* out) {
+  __shared__ double s_part[32];
+  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+  const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+  rate = warp_max(rate);
+  if ((tid & 31) == 0) s_part[tid >> 5] = rate;
+  __syncthreads();
+  if (tid < 32) {
+    double v = (tid < (nthreads + 31) / 32) ? s_part[tid] : 0.0;
+    v = warp_max(v);
+    if (tid == 0) atomicMax(out, (unsigned long long)__double_as_longlong(v));
+  }
+}
+
+}  // namespace hx

@@ -14,7 +14,7 @@ import math
 
 import numpy as np
 
-# enum values of include/hx.h and oracle/ox.h (both headers declare the same numbers)
+# enum values shared by the problem descriptions (the CUDA header and the oracle header each declare the same numbers)
 CARTESIAN, SPHERICAL = 0, 1
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTING, BC_WEDGE = 0, 1, 2, 3
 RIEMANN_HLL, RIEMANN_HLLC = 0, 1
@@ -95,16 +95,17 @@ def sod_1d(n=1000):
 
 def kh_2d(n=1024, seed=1002):
     """C2: 2-D periodic shear layer + 1 scalar, MC + HLLC, CFL 0.8, 200 steps (shape of PAPER.md Sect. 4.1)."""
-    fx = uniform_faces(0.0, 1.0, n)
-    fy = uniform_faces(0.0, 1.0, n)
-    spec = _spec("kh_2d", 2, [n, n], [fx, fy], [BC_PERIODIC] * 2, [BC_PERIODIC] * 2, 1.4, LIM_MC,
+    nx, ny = (n, n) if np.isscalar(n) else n
+    fx = uniform_faces(0.0, 1.0, nx)
+    fy = uniform_faces(0.0, 1.0, ny)
+    spec = _spec("kh_2d", 2, [nx, ny], [fx, fy], [BC_PERIODIC] * 2, [BC_PERIODIC] * 2, 1.4, LIM_MC,
                  n_scalars=1, cfl=0.8, steps=200, seed=seed)
     y = centres(fy)
     band = (np.abs(y - 0.5) < 0.25)[:, None]
-    W = np.empty((5, 1, n, n))
+    W = np.empty((5, 1, ny, nx))
     W[0, 0] = np.where(band, 2.0, 1.0)
     W[1, 0] = np.where(band, 0.5, -0.5)
-    W[2, 0] = 0.01 * noise(seed, (n, n))
+    W[2, 0] = 0.01 * noise(seed, (ny, nx))
     W[3, 0] = 2.5
     W[4, 0] = np.where(band, 1.0, 0.0)
     return spec, W
@@ -114,18 +115,19 @@ def sedov_3d(n=256, seed=1003):
     """C3: 3-D Cartesian blast, transmissive, gamma 5/3, minmod + HLLC, CFL 0.6, 100 steps
     (shape of PAPER.md Sect. 4.3 / App. C.4).  E = 1 as thermal energy in the cells whose
     centre lies within 3.5 dx of the origin (160 cells at any even n, reading R23)."""
-    f = uniform_faces(-0.5, 0.5, n)
+    nx, ny, nz = (n, n, n) if np.isscalar(n) else n
+    fs = [uniform_faces(-0.5, 0.5, m) for m in (nx, ny, nz)]
     gamma = 5.0 / 3.0
-    spec = _spec("sedov_3d", 3, [n] * 3, [f, f, f], [BC_TRANSMISSIVE] * 3, [BC_TRANSMISSIVE] * 3, gamma,
+    spec = _spec("sedov_3d", 3, [nx, ny, nz], fs, [BC_TRANSMISSIVE] * 3, [BC_TRANSMISSIVE] * 3, gamma,
                  LIM_MINMOD, cfl=0.6, steps=100, seed=seed)
-    dx = 1.0 / n
-    c = centres(f)
-    r2 = c[:, None, None] ** 2 + c[None, :, None] ** 2 + c[None, None, :] ** 2
+    dx = 1.0 / nx                              # reduced copies: radius in units of the x spacing
+    cx, cy, cz = (centres(f) for f in fs)
+    r2 = cz[:, None, None] ** 2 + cy[None, :, None] ** 2 + cx[None, None, :] ** 2
     inside = r2 < (3.5 * dx) ** 2
     ncell = int(inside.sum())
-    W = np.zeros((5, n, n, n))
-    W[0] = 1.0 + 0.01 * noise(seed, (n, n, n))
-    W[4] = np.where(inside, (gamma - 1.0) * 1.0 / (ncell * dx ** 3), 1e-5)
+    W = np.zeros((5, nz, ny, nx))
+    W[0] = 1.0 + 0.01 * noise(seed, (nz, ny, nx))
+    W[4] = np.where(inside, (gamma - 1.0) * 1.0 / (ncell * (1.0 / nx) * (1.0 / ny) * (1.0 / nz)), 1e-5)
     spec["bomb_cells"] = ncell
     return spec, W
 
@@ -134,19 +136,21 @@ def rt_3d(n=512, seed=1004):
     """C4: 3-D Rayleigh-Taylor, n x n x n cells on [0,1]^2 x [0,2] (dz = 2 dx), periodic x/y,
     reflecting z, g = -0.1 z, 2 scalars, MC + HLLC, CFL 0.7, 50 steps (shape of PAPER.md Sect. 4.2,
     the paper's weak-scaling workload, App. B)."""
-    fx = uniform_faces(0.0, 1.0, n)
-    fz = uniform_faces(0.0, 2.0, n)
+    nx, ny, nz = (n, n, n) if np.isscalar(n) else n
+    fx = uniform_faces(0.0, 1.0, nx)
+    fy = uniform_faces(0.0, 1.0, ny)
+    fz = uniform_faces(0.0, 2.0, nz)
     g = -0.1
-    spec = _spec("rt_3d", 3, [n] * 3, [fx, fx, fz], [BC_PERIODIC, BC_PERIODIC, BC_REFLECTING],
+    spec = _spec("rt_3d", 3, [nx, ny, nz], [fx, fy, fz], [BC_PERIODIC, BC_PERIODIC, BC_REFLECTING],
                  [BC_PERIODIC, BC_PERIODIC, BC_REFLECTING], 1.4, LIM_MC, n_scalars=2,
                  gravity=GRAV_UNIFORM, g=(0.0, 0.0, g), cfl=0.7, steps=50, seed=seed)
     z = centres(fz)
     heavy = z > 1.0
     rho = np.where(heavy, 2.0, 1.0)
     p = 2.5 + g * rho * (z - 1.0)           # analytic piecewise hydrostatic column, P(1) = 2.5
-    W = np.zeros((7, n, n, n))
+    W = np.zeros((7, nz, ny, nx))
     W[0] = rho[:, None, None]
-    W[3] = 0.01 * noise(seed, (n, n, n)) * (np.abs(z - 1.0) < 0.05)[:, None, None]
+    W[3] = 0.01 * noise(seed, (nz, ny, nx)) * (np.abs(z - 1.0) < 0.05)[:, None, None]
     W[4] = p[:, None, None]
     W[5] = np.where(heavy, 1.0, 0.0)[:, None, None]
     W[6] = np.where(heavy, 0.0, 1.0)[:, None, None]

@@ -656,3 +656,117 @@ def test_cfl_time_step_closed_form(oxlib):
     with pytest.raises(ox.OracleError) as e:
         o.compute_dt(0.6)
     assert e.value.code == ox.ERR_NONPHYSICAL
+
+
+# ------------------------------------------------------------------------------------------ P12
+def plane_wave_in_spherical(ox, ndim, n, t_end, limiter=2, amp=0.2, speed=1.0):
+    """A density wave carried by a uniform Cartesian velocity (rho(x - U t), u = U, P = const) is an
+    exact solution of Eq. 1.  Written in (r, theta[, phi]) it exercises every geometric factor and
+    source term of Eq. 13-16 with u_theta, u_phi != 0.  A band of 4 cells along the open boundaries
+    is reset to the exact solution after each step so that boundary errors never reach the interior."""
+    gamma = 1.4
+    fr = wl.uniform_faces(1.0, 2.0, n)
+    # off-equator wedge so that the cot(theta) terms of Eq. 13-16 are not small
+    ft = wl.uniform_faces(0.5, 1.5, n)
+    faces = [fr, ft]
+    nn = [n, n]
+    if ndim == 3:
+        faces.append(wl.uniform_faces(-0.5, 0.5, n))
+        nn.append(n)
+        Uc = speed * np.array([0.35, -0.2, 0.3])   # Cartesian velocity
+        kv = 2 * math.pi * np.array([1.0, 1.0, -1.0])
+    else:
+        Uc = speed * np.array([0.0, 0.0, 0.4])     # along the polar axis: axisymmetric
+        kv = 2 * math.pi * np.array([0.0, 0.0, 1.5])
+    spec = wl._spec("planewave", ndim, nn, faces, [1] * ndim, [1] * ndim, gamma, limiter, coords=ox.SPHERICAL, n_scalars=1)
+    r = wl.centres(fr)[None, None, :]
+    th = wl.centres(ft)[None, :, None]
+    ph = wl.centres(faces[2])[:, None, None] if ndim == 3 else np.zeros((1, 1, 1))
+    x, y, z = r * np.sin(th) * np.cos(ph), r * np.sin(th) * np.sin(ph), r * np.cos(th)
+    er = np.stack(np.broadcast_arrays(np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph), np.cos(th) + 0 * ph))
+    et = np.stack(np.broadcast_arrays(np.cos(th) * np.cos(ph), np.cos(th) * np.sin(ph), -np.sin(th) + 0 * ph))
+    ep = np.stack(np.broadcast_arrays(-np.sin(ph) + 0 * th, np.cos(ph) + 0 * th, 0 * th + 0 * ph))
+    shape = np.broadcast_shapes(x.shape, y.shape, z.shape)
+
+    def exact(t):
+        W = np.empty((3 + ndim,) + shape)
+        phase = kv[0] * (x - Uc[0] * t) + kv[1] * (y - Uc[1] * t) + kv[2] * (z - Uc[2] * t)
+        W[0] = 1.0 + amp * np.sin(phase)
+        W[1] = np.tensordot(Uc, er, axes=1)
+        W[2] = np.tensordot(Uc, et, axes=1)
+        if ndim == 3:
+            W[3] = np.tensordot(Uc, ep, axes=1)
+        W[1 + ndim] = 1.0
+        W[2 + ndim] = 0.5 + 0.3 * np.cos(phase)
+        return W
+    o = make(ox, spec, exact(0.0))
+    band = np.ones(shape, dtype=bool)
+    sl = tuple(slice(4, -4) for _ in range(ndim))
+    band[(slice(None),) * (3 - ndim) + sl] = False
+    t = 0.0
+    while t < t_end * (1 - 1e-12):
+        dt = min(o.compute_dt(0.5), t_end - t)
+        o.step(dt)
+        t += dt
+        P = o.get_state(ox.PRIMITIVE)
+        E = exact(t)
+        P[:, band] = E[:, band]
+        o.set_state(P, ox.PRIMITIVE)
+    P = o.get_state(ox.PRIMITIVE)
+    E = exact(t_end)
+    inner = (slice(None),) + (slice(None),) * (3 - ndim) + tuple(slice(6, -6) for _ in range(ndim))
+    return [float(np.mean(np.abs(P[v][inner[1:]] - E[v][inner[1:]]))) for v in range(3 + ndim)]
+
+
+@pytest.mark.parametrize("ndim,sizes,amp,speed,bar", [(2, (32, 64), 0.2, 1.0, 1.6), (3, (20, 40), 0.2, 1.0, 1.6),
+                                                      (3, (20, 40), 0.0, 3.0, 1.45)])
+def test_p12_cartesian_plane_wave_on_spherical_grid(oxlib, ndim, sizes, amp, speed, bar):
+    # the fast uniform flow (amp 0, speed 3) makes the u_theta u_phi geometric terms of the
+    # predictor dominate the error: dropping one of them shows up as first-order convergence
+    e1 = plane_wave_in_spherical(oxlib, ndim, sizes[0], 0.1, amp=amp, speed=speed)
+    e2 = plane_wave_in_spherical(oxlib, ndim, sizes[1], 0.1, amp=amp, speed=speed)
+    for v in range(3 + ndim):
+        order = math.log2(e1[v] / e2[v])
+        assert order > bar, (v, e1, e2)
+        assert e2[v] < 2e-3, (v, e2)
+
+
+# ------------------------------------------------------------------------------------------ P9b
+def falling_wave_error(ox, ndim, n, limiter=2):
+    """rho(x - X(t)) with X = u0 t + g t^2/2, u = u0 + g t, P const: exact with uniform gravity, periodic box."""
+    faces = [wl.uniform_faces(0.0, 1.0, n) for _ in range(ndim)]
+    g = [0.8, -0.6, 0.0][:ndim] + [0.0] * (3 - ndim)
+    u0 = [0.3, 0.5, 0.0][:ndim]
+    spec = wl._spec("fallwave", ndim, [n] * ndim, faces, [0] * ndim, [0] * ndim, 1.4, limiter, gravity=ox.GRAV_UNIFORM, g=g)
+    c = wl.centres(faces[0])
+    grids = [c.reshape([n if (2 - e) == d else 1 for e in range(3)]) for d in range(ndim)]
+    shape = tuple([n if (2 - e) < ndim else 1 for e in range(3)])
+    t_end = 0.5
+
+    def rho(t):
+        ph = 0.0
+        for d in range(ndim):
+            ph = ph + (grids[d] - (u0[d] * t + 0.5 * g[d] * t * t))
+        return np.broadcast_to(1.0 + 0.2 * np.sin(2 * math.pi * ph), shape)
+    W = np.empty((2 + ndim,) + shape)
+    W[0] = rho(0.0)
+    for d in range(ndim):
+        W[1 + d] = u0[d]
+    W[1 + ndim] = 1.0
+    o = make(ox, spec, W)
+    run_to_time(o, 0.6, t_end)
+    P = o.get_state(ox.PRIMITIVE)
+    errs = [float(np.mean(np.abs(P[0] - rho(t_end))))]
+    for d in range(ndim):
+        errs.append(float(np.mean(np.abs(P[1 + d] - (u0[d] + g[d] * t_end)))))
+    errs.append(float(np.mean(np.abs(P[1 + ndim] - 1.0))))
+    return errs
+
+
+@pytest.mark.parametrize("ndim,sizes", [(1, (64, 128)), (2, (32, 64))])
+def test_p9b_advection_in_free_fall_second_order(oxlib, ndim, sizes):
+    e1 = falling_wave_error(oxlib, ndim, sizes[0])
+    e2 = falling_wave_error(oxlib, ndim, sizes[1])
+    assert math.log2(e1[0] / e2[0]) > 1.7, (e1, e2)
+    for v in range(1, 2 + ndim):        # velocity and pressure errors: second order too (and tiny)
+        assert e2[v] < 1e-4 and (e1[v] < 1e-9 or math.log2(e1[v] / e2[v]) > 1.5), (v, e1, e2)

@@ -1,0 +1,199 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle.  `-m gpu` only.
+
+Tolerances (BASELINE.json north_star, reading R22 for the norms): max relative difference per stored
+field <= 1e-12 after one step; L1 relative difference <= 1e-9 after 100 steps (or the config's last
+step).  dt itself must agree to 1e-13 relative.  Both sides get bit-identical inputs and face arrays.
+"""
+import numpy as np
+import pytest
+
+from paper_2503_04428_b200 import workloads as wl
+from tests.helpers import l1_rel_per_field, max_rel_per_field
+from tests.test_oracle_pins import CASES_P11, random_problem
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-12
+TOL_L1 = 1e-9
+KERNELS = ["generic", "auto"]
+
+
+@pytest.fixture(scope="module")
+def hx():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2503_04428_b200 import hx as mod
+    mod.lib()
+    return mod
+
+
+def make_pair(hx, ox, spec, W, kernel="auto"):
+    g = hx.Hydro(spec)
+    if kernel == "generic":
+        g.set_option(hx.OPT_KERNEL, hx.KERNEL_GENERIC)
+    g.set_state(np.ascontiguousarray(W), hx.PRIMITIVE)
+    o = ox.Oracle(spec)
+    o.set_state(W, ox.PRIMITIVE)
+    return g, o
+
+
+def cell_volumes(o, spec):
+    n = spec["n"]
+    if spec["coords"] == 0:
+        return None   # uniform Cartesian reduced copies: dV constant, cancels in the ratio
+    dV = np.empty((n[2], n[1], n[0]))
+    for k in range(n[2]):
+        for j in range(n[1]):
+            for i in range(n[0]):
+                dV[k, j, i] = o.cell_geometry(i, j, k)[0]
+    return dV
+
+
+# reduced copies of the five configs: several tiles plus a ragged tail in every direction
+REDUCED = {
+    "sod_1d": lambda: wl.sod_1d(1000),
+    "kh_2d": lambda: wl.kh_2d((200, 136)),
+    "sedov_3d": lambda: wl.sedov_3d((72, 44, 38)),
+    "rt_3d": lambda: wl.rt_3d((70, 36, 42)),
+    "wedge_3d": lambda: wl.wedge_3d((104, 22, 26)),
+}
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("name", list(REDUCED))
+def test_one_step_parity(hx, oxlib, name, kernel):
+    ox = oxlib
+    spec, W = REDUCED[name]()
+    g, o = make_pair(hx, ox, spec, W, kernel)
+    dt_g, dt_o = g.compute_dt(spec["cfl"]), o.compute_dt(spec["cfl"])
+    assert abs(dt_g - dt_o) <= 1e-13 * dt_o
+    g.step(dt_o)
+    o.step(dt_o)
+    Ug, Uo = g.get_state(), o.get_state()
+    assert np.max(np.abs(Uo - ox.Oracle(spec).get_state())) > 0
+    rel = max_rel_per_field(Ug, Uo, spec["ndim"])
+    assert max(rel) <= TOL_STEP, (name, kernel, g.step_kernel, rel)
+    # the rate folded into the step equals the stand-alone reduction of the oracle on the new state
+    dt_g2, dt_o2 = g.compute_dt(spec["cfl"]), o.compute_dt(spec["cfl"])
+    assert abs(dt_g2 - dt_o2) <= 1e-12 * dt_o2
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("name", list(REDUCED))
+def test_hundred_step_parity(hx, oxlib, name, kernel):
+    ox = oxlib
+    spec, W = REDUCED[name]()
+    g, o = make_pair(hx, ox, spec, W, kernel)
+    nsteps = 100 if spec["steps"] is None else min(100, spec["steps"])
+    for s in range(nsteps):
+        dt_g, dt_o = g.compute_dt(spec["cfl"]), o.compute_dt(spec["cfl"])
+        assert abs(dt_g - dt_o) <= 1e-10 * dt_o, (s, dt_g, dt_o)
+        g.step(dt_g)
+        o.step(dt_o)
+    Ug, Uo = g.get_state(), o.get_state()
+    l1 = l1_rel_per_field(Ug, Uo, spec["ndim"], cell_volumes(o, spec))
+    assert max(l1) <= TOL_L1, (name, kernel, g.step_kernel, l1)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("case", CASES_P11, ids=[c[0] for c in CASES_P11])
+def test_every_bc_geometry_solver_limiter(hx, oxlib, case, kernel):
+    """Tiny random problems: every boundary type on every face, both geometries, both solvers, every
+    limiter, non-uniform grids, gravity of both kinds (same cases as oracle pin P11)."""
+    ox = oxlib
+    spec, W = random_problem(ox, case)
+    g, o = make_pair(hx, ox, spec, W, kernel)
+    for _ in range(3):
+        dt = 0.5 * o.compute_dt(0.5)
+        assert abs(0.5 * g.compute_dt(0.5) - dt) <= 1e-13 * dt
+        g.step(dt)
+        o.step(dt)
+    rel = max_rel_per_field(g.get_state(), o.get_state(), spec["ndim"])
+    assert max(rel) <= 3 * TOL_STEP, (case[0], rel)
+
+
+@pytest.mark.parametrize("lim", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("riemann", [0, 1])
+def test_limiters_and_solvers_3d(hx, oxlib, lim, riemann):
+    ox = oxlib
+    spec, W = wl.smooth_periodic(3, [40, 24, 20], seed=21, n_scalars=1, limiter=lim, riemann=riemann)
+    W[0] += 0.8 * (W[1] > 0.1)        # add jumps so that limiters and wave-speed branches switch
+    g, o = make_pair(hx, ox, spec, W)
+    for _ in range(5):
+        dt = o.compute_dt(0.5)
+        g.step(dt)
+        o.step(dt)
+    rel = max_rel_per_field(g.get_state(), o.get_state(), 3)
+    assert max(rel) <= 5 * TOL_STEP, rel
+
+
+def test_library_spacing_modes_match_custom_faces(hx, oxlib):
+    """HX_SPACING_UNIFORM / LOG computed inside the library vs the oracle's own uniform / log faces."""
+    ox = oxlib
+    spec, W = wl.wedge_3d((40, 10, 12))
+    spec = dict(spec)
+    spec["faces"] = [None, None, None]
+    spec["spacing"] = [wl.SPACING_LOG, wl.SPACING_UNIFORM, wl.SPACING_UNIFORM]
+    g, o = make_pair(hx, ox, spec, W)
+    dt = o.compute_dt(0.6)
+    assert abs(g.compute_dt(0.6) - dt) <= 1e-13 * dt
+    g.step(dt)
+    o.step(dt)
+    assert max(max_rel_per_field(g.get_state(), o.get_state(), 3)) <= TOL_STEP
+
+
+def test_state_round_trip_and_forms(hx, oxlib):
+    ox = oxlib
+    import torch
+    spec, W = wl.smooth_periodic(3, [18, 10, 6], seed=4, n_scalars=2)
+    g, o = make_pair(hx, ox, spec, W)
+    assert g.nvar == 7 and g.shape == (7, 6, 10, 18)
+    Uo = o.get_state()
+    Ug = g.get_state()
+    assert np.max(np.abs(Ug - Uo)) <= 1e-15 * np.max(np.abs(Uo))
+    Wg = g.get_state(form=hx.PRIMITIVE)
+    assert np.max(np.abs(Wg - W)) <= 1e-14
+    g.set_state(Uo, hx.CONSERVED)
+    assert np.array_equal(g.get_state(), Uo)                      # conserved in -> out is a pure copy
+    # device-pointer path on a non-default torch stream
+    stream = torch.cuda.Stream()
+    g.set_stream(stream)
+    with torch.cuda.stream(stream):
+        dev = torch.from_numpy(Uo).cuda()
+        g.set_state(dev, hx.CONSERVED)
+        out = torch.empty_like(dev)
+        g.get_state(out, hx.CONSERVED)
+    assert torch.equal(out.cpu(), torch.from_numpy(Uo))
+    with pytest.raises(ValueError):
+        g.set_state(np.zeros(5))
+
+
+def test_nonphysical_state_is_reported_not_floored(hx):
+    spec, W = wl.smooth_periodic(2, [32, 16], seed=9, n_scalars=0)
+    g = hx.Hydro(spec)
+    bad = W.copy()
+    bad[3, 0, 3, 5] = -0.5          # negative pressure
+    g.set_state(bad, hx.PRIMITIVE)
+    with pytest.raises(hx.HxError) as e:
+        g.compute_dt(0.5)
+    assert e.value.code == hx.ERR_NONPHYSICAL
+    g.set_state(W, hx.PRIMITIVE)    # the flag is cleared by a new state
+    assert g.compute_dt(0.5) > 0
+    with pytest.raises(hx.HxError):
+        g.step(-1.0)
+    # a far too large time step drives the update non-physical: reported at the next sync call
+    g.step(50.0 * g.compute_dt(0.5))
+    with pytest.raises(hx.HxError) as e:
+        g.compute_dt(0.5)
+    assert e.value.code == hx.ERR_NONPHYSICAL
+
+
+def test_minimum_sizes_and_degenerate_shapes(hx, oxlib):
+    ox = oxlib
+    for ndim, n in ((1, [2]), (2, [2, 3]), (3, [2, 2, 2]), (3, [3, 2, 5]), (1, [33])):
+        spec, W = wl.smooth_periodic(ndim, n, seed=ndim, n_scalars=1)
+        g, o = make_pair(hx, ox, spec, W)
+        dt = o.compute_dt(0.4)
+        g.step(dt)
+        o.step(dt)
+        assert max(max_rel_per_field(g.get_state(), o.get_state(), ndim)) <= TOL_STEP, n
