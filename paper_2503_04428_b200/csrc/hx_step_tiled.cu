@@ -701,6 +701,8 @@ cudaError_t tiled_plan_create(const Layout& L, const Phys&, double* const U[2], 
   p->ty = TY_DEFAULT;
   const int ntx = (L.n[0] + TXMAX - 1) / TXMAX, nty = (L.n[1] + p->ty - 1) / p->ty;
   p->wx = (L.n[0] + ntx - 1) / ntx;
+  p->wx += p->wx & 1;   // even tile width: with the even `lead` every TMA box then starts on a 16-byte boundary
+                        // (an odd start coordinate of this fp64 box raises "illegal instruction" on sm_100a)
   p->wy = (L.n[1] + nty - 1) / nty;
   // z chunks: enough CTAs for >= ~6 waves over 148 SMs, chunks of at least 16 planes (2 warm-up planes each)
   int nzc = 1;

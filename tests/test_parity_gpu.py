@@ -197,3 +197,19 @@ def test_minimum_sizes_and_degenerate_shapes(hx, oxlib):
         g.step(dt)
         o.step(dt)
         assert max(max_rel_per_field(g.get_state(), o.get_state(), ndim)) <= TOL_STEP, n
+
+
+@pytest.mark.parametrize("n", [(58, 20, 18), (87, 12, 8), (31, 11, 5), (30, 10, 16), (61, 21, 33)])
+def test_tile_edges_and_odd_widths(hx, oxlib, n):
+    """Grid widths that give odd balanced tile widths (58 -> 2 x 29), exactly full tiles, and one
+    cell more than a full tile, in x and y; z chunk boundaries.  (An odd TMA start coordinate of the
+    fp64 box is illegal on sm_100a: the plan must round tile widths to even.)"""
+    ox = oxlib
+    spec, W = wl.smooth_periodic(3, list(n), seed=n[0], n_scalars=0, limiter=wl.LIM_MC)
+    g, o = make_pair(hx, ox, spec, W, "auto")
+    for _ in range(2):
+        dt = o.compute_dt(0.5)
+        g.step(dt)
+        o.step(dt)
+    assert g.step_kernel == "tiled3d"
+    assert max(max_rel_per_field(g.get_state(), o.get_state(), 3)) <= 2 * TOL_STEP, n
