@@ -47,6 +47,22 @@ WORKLOADS = {
 DEFAULT_WORKLOAD = "rt_3d"
 
 
+def alg_flops_per_cell(spec):
+    """Algorithmic fp64 flops per 3-D cell-update (hand count from O1-O7 with every
+    predictor and face flux computed once; + and x count 1 each, so an FMA is 2; div and sqrt 1 each):
+    629 for nvar = 5, HLLC/HLL + minmod; +4 per slope for MC / van Leer, +6 van Albada; +84 per passive
+    scalar; +31 gravity; +65 spherical sources."""
+    ns = spec["nvar"] - 2 - spec["ndim"]
+    nvar = spec["nvar"]
+    lim_extra = {wl.LIM_NONE: -1, wl.LIM_MINMOD: 0, wl.LIM_VANLEER: 4, wl.LIM_VANALBADA: 6, wl.LIM_MC: 4}[spec["limiter"]]
+    f = 629 + 84 * ns + 3 * nvar * lim_extra
+    if spec["gravity"] != wl.GRAV_NONE:
+        f += 31
+    if spec["coords"] == wl.SPHERICAL:
+        f += 65
+    return f
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -262,6 +278,9 @@ def run_ours(args):
             traffic = json.load(open(tpath)).get(args.workload, {}).get(kernel_name)
         except Exception:
             traffic = None
+    fp64_peak, dfma_lat = hx.probe_fp64()              # measured FP64 FMA rate of this GPU (TFLOP/s) and DFMA latency
+    alg_flops = alg_flops_per_cell(spec) * ncell
+    alu_achieved = alg_flops / (kernel_ms * 1e-3) / 1e12
     cpu_val, cpu_sample, cores, _ = time_oracle(make_reduced, budget_s=args.cpu_budget)
     state_gb = 2 * nvar * ncell * 8 / 1e9
     out = {
@@ -273,9 +292,14 @@ def run_ours(args):
                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no sharding, SURVEY 8(e))",
                    "l2": f"inputs larger than L2 (two state buffers = {state_gb:.1f} GB vs 126 MB L2)" if state_gb > 0.5
                          else "state fits in L2: HBM fraction not meaningful for this workload"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "kernel": kernel_name, "kernel_ms": kernel_ms, "algorithmic_bytes_per_launch": alg_bytes,
-                     "peak_source": peak_src, "kernel_share_of_step": kernel_ms / (total_ms / K)},
+        # the path is FP64-pipe bound on B200: the binding roof is "alu"; the HBM figures stay beside it
+        "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": alu_achieved / fp64_peak,
+                     "traffic": traffic, "kernel": kernel_name, "kernel_ms": kernel_ms,
+                     "algorithmic_flops_per_cell": alg_flops_per_cell(spec), "algorithmic_flops_per_launch": alg_flops,
+                     "peak_source": "measured on this GPU by hx_probe_fp64 (independent DFMA chains on all SMs; nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2)",
+                     "dfma_dependent_latency_cycles": dfma_lat, "kernel_share_of_step": kernel_ms / (total_ms / K)},
+        "roofline_hbm": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src},
         "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_sample},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},

@@ -100,6 +100,10 @@ int hx_kernel_time(hx_handle* h, double* total_ms, long long* launches);
 /* Name of the step kernel the last hx_step used ("generic", "tiled3d", ..). */
 const char* hx_step_kernel_name(const hx_handle* h);
 const char* hx_last_error(const hx_handle* h);
+/* Device probe (no handle, default stream, synchronous): measured FP64 FMA throughput of the current
+ * GPU in TFLOP/s (1 FMA = 2 flop; many independent chains on every SM) and the issue-to-issue latency
+ * of a dependent DFMA in SM cycles.  This is the denominator of the "alu" roofline. */
+int hx_probe_fp64(double* tflops, double* dep_latency_cycles);
 const char* hx_version(void);
 
 #ifdef __cplusplus

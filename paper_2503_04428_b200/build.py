@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libhx.so")
-SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_step_tiled.cu"]
+SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_step_tiled.cu", "hx_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -27,7 +27,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 EXPORTS = ["hx_create", "hx_destroy", "hx_set_stream", "hx_set_option", "hx_set_state", "hx_get_state",
            "hx_compute_dt", "hx_step", "hx_nvar", "hx_launch_count", "hx_kernel_time", "hx_step_kernel_name", "hx_last_error",
-           "hx_version"]
+           "hx_version", "hx_probe_fp64"]
 
 
 class HxConfig(C.Structure):
@@ -81,6 +81,7 @@ def lib():
         L.hx_last_error.argtypes = [vp]
         L.hx_last_error.restype = C.c_char_p
         L.hx_version.restype = C.c_char_p
+        L.hx_probe_fp64.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -206,6 +207,15 @@ class Hydro:
     @property
     def step_kernel(self) -> str:
         return self._L.hx_step_kernel_name(self._h).decode()
+
+
+def probe_fp64():
+    """(measured FP64 FMA throughput in TFLOP/s, dependent-DFMA latency in cycles) of the current GPU."""
+    tf, lat = C.c_double(), C.c_double()
+    rc = lib().hx_probe_fp64(C.byref(tf), C.byref(lat))
+    if rc != OK:
+        raise HxError(rc, "hx_probe_fp64")
+    return tf.value, lat.value
 
 
 def version() -> str:
