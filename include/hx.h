@@ -43,7 +43,8 @@ enum { HX_CONSERVED = 0, HX_PRIMITIVE = 1 };
 /* Step kernel selection (hx_set_option(HX_OPT_KERNEL, ..)): AUTO picks the fused tile kernel where
  * it applies and the generic one elsewhere; the other two force one path (tests, profiling). */
 enum { HX_OPT_KERNEL = 0, HX_OPT_TIMING = 1 /* 0/1: bracket each step-kernel launch with CUDA events */ };
-enum { HX_KERNEL_AUTO = 0, HX_KERNEL_GENERIC = 1, HX_KERNEL_TILED = 2 };
+enum { HX_KERNEL_AUTO = 0, HX_KERNEL_GENERIC = 1, HX_KERNEL_TILED = 2 /* first tiled design, kept for A/B runs */,
+       HX_KERNEL_TILE2 = 3 /* ring-warp tile kernel, what AUTO picks in 3-D */ };
 
 #define HX_MAX_NVAR 16
 

@@ -22,6 +22,12 @@ cudaError_t tiled_plan_create(const Layout& L, const Phys& P, double* const U[2]
 void tiled_plan_destroy(TiledPlan* p);
 cudaError_t launch_step_tiled(TiledPlan* plan, const StepArgs& a, int cur, cudaStream_t s);
 const char* tiled_kernel_name(const TiledPlan* p);
+namespace t2 { struct Plan; }
+int tile2_supported(const Layout& L, const Phys& P);
+cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, t2::Plan** out);
+void tile2_plan_destroy(t2::Plan* p);
+cudaError_t launch_step_tile2(t2::Plan* plan, const StepArgs& a, int cur, cudaStream_t s);
+const char* tile2_kernel_name(const t2::Plan* p);
 }  // namespace hx
 
 using namespace hx;
@@ -47,6 +53,10 @@ struct hx_handle {
   int kernel_opt = HX_KERNEL_AUTO;
   TiledPlan* plan = nullptr;
   bool plan_tried = false;
+  t2::Plan* plan2 = nullptr;
+  bool plan2_tried = false;
+  bool uniform = false;       // Cartesian grid whose per-axis tables are bitwise constant
+  double uni[6] = {0, 0, 0, 0, 0, 0};   // hw*idx and 1/delta of the three axes when uniform
   long long launches = 0;
   const char* last_kernel = "none";
   bool timing = false, ev_pending = false;
@@ -227,6 +237,18 @@ int build_tables(hx_handle* h) {
     for (int p = 0; p < L.np[2]; ++p) pool[idphi + p] = 1.0 / (xf[2][p + 1] - xf[2][p]);
   }
 
+  // Bitwise-uniform Cartesian grid (e.g. 2^k cells on a dyadic extent): every cell of an axis has the same
+  // hw, 1/width and 1/(centre distance), so the step kernel may take them as constants without changing a bit.
+  h->uniform = !sph && c.ndim == 3;
+  for (int d = 0; d < 3 && h->uniform; ++d) {
+    for (int p = 1; p < L.np[d]; ++p)
+      if (memcmp(&pool[hw[d] + p], &pool[hw[d]], 8) || memcmp(&pool[iw[d] + p], &pool[iw[d]], 8) ||
+          memcmp(&pool[idx[d] + p], &pool[idx[d] + 1], 8))
+        h->uniform = false;
+    h->uni[d] = pool[hw[d] + 1] * pool[idx[d] + 1];
+    h->uni[3 + d] = pool[iw[d] + 1];
+  }
+
   const size_t bytes = pool.size() * sizeof(double);
   cudaError_t e = cudaMalloc(&h->d_tables, bytes);
   if (e != cudaSuccess) return cuda_fail(h, e, "cudaMalloc(tables)");
@@ -352,6 +374,7 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
 int hx_destroy(hx_handle* h) {
   if (!h) return HX_OK;
   if (h->plan) tiled_plan_destroy(h->plan);
+  if (h->plan2) tile2_plan_destroy(h->plan2);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   for (int b = 0; b < 2; ++b)
@@ -372,8 +395,9 @@ int hx_set_stream(hx_handle* h, void* cuda_stream) {
 int hx_set_option(hx_handle* h, int option, int value) {
   if (!h) return HX_ERR_INVALID_ARG;
   if (option == HX_OPT_KERNEL) {
-    if (value < HX_KERNEL_AUTO || value > HX_KERNEL_TILED) return fail(h, HX_ERR_INVALID_ARG, "unknown kernel selection");
+    if (value < HX_KERNEL_AUTO || value > HX_KERNEL_TILE2) return fail(h, HX_ERR_INVALID_ARG, "unknown kernel selection");
     if (value == HX_KERNEL_TILED && !tiled_supported(h->L, h->P)) return fail(h, HX_ERR_UNSUPPORTED, "the tiled kernel does not cover this configuration");
+    if (value == HX_KERNEL_TILE2 && !tile2_supported(h->L, h->P)) return fail(h, HX_ERR_UNSUPPORTED, "the tile2 kernel does not cover this configuration");
     h->kernel_opt = value;
     return HX_OK;
   }
@@ -485,23 +509,38 @@ int hx_step(hx_handle* h, double dt) {
   e = cudaMemsetAsync(&h->d_scal->rate_bits, 0, sizeof(unsigned long long), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: memset");
   StepArgs a = make_args(h, dt);
-  bool use_tiled = false;
-  if (h->kernel_opt != HX_KERNEL_GENERIC && tiled_supported(L, h->P)) {
+  bool use_tiled = false, use_tile2 = false;
+  const int ko = h->kernel_opt;
+  if ((ko == HX_KERNEL_AUTO || ko == HX_KERNEL_TILE2) && tile2_supported(L, h->P)) {
+    if (!h->plan2 && !h->plan2_tried) {
+      h->plan2_tried = true;
+      const int grav_z = h->cfg.gravity == HX_GRAV_UNIFORM && h->cfg.g[0] == 0.0 && h->cfg.g[1] == 0.0;
+      e = tile2_plan_create(L, h->P, h->d_U, h->uniform ? h->uni : nullptr, grav_z, &h->plan2);
+      if (e != cudaSuccess) {
+        h->plan2 = nullptr;
+        return cuda_fail(h, e, "hx_step: tile2 plan");   // no silent fallback to a slower path
+      }
+    }
+    use_tile2 = h->plan2 != nullptr;
+    if (!use_tile2) return fail(h, HX_ERR_CUDA, "tile2 kernel unavailable");
+  } else if (ko == HX_KERNEL_TILED && tiled_supported(L, h->P)) {
     if (!h->plan && !h->plan_tried) {
       h->plan_tried = true;
       e = tiled_plan_create(L, h->P, h->d_U, &h->plan);
       if (e != cudaSuccess) {
         h->plan = nullptr;
-        if (h->kernel_opt == HX_KERNEL_TILED) return cuda_fail(h, e, "hx_step: tiled plan");
-        cudaGetLastError();
+        return cuda_fail(h, e, "hx_step: tiled plan");
       }
     }
     use_tiled = h->plan != nullptr;
-    if (!use_tiled && h->kernel_opt == HX_KERNEL_TILED) return fail(h, HX_ERR_CUDA, "tiled kernel unavailable");
+    if (!use_tiled) return fail(h, HX_ERR_CUDA, "tiled kernel unavailable");
   }
   const bool timed = h->timing && !h->ev_pending;
   if (timed) cudaEventRecord(h->ev0, h->stream);
-  if (use_tiled) {
+  if (use_tile2) {
+    e = launch_step_tile2(h->plan2, a, h->cur, h->stream);
+    h->last_kernel = tile2_kernel_name(h->plan2);
+  } else if (use_tiled) {
     e = launch_step_tiled(h->plan, a, h->cur, h->stream);
     h->last_kernel = tiled_kernel_name(h->plan);
   } else {

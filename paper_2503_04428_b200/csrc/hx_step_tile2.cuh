@@ -1,0 +1,674 @@
+// hx_step_tile2.cuh -- the fused 3-D step kernel, second design (A1-A7 of SURVEY 8(a) in ONE pass over HBM).
+//
+// Why a second design: ncu on the first tiled kernel (profiles/r1a_*) showed the FP64 pipe only half
+// busy with the issue port just as loaded (fp64 : other instructions = 1 : 1), 22 % of the threads
+// doing full work on ring cells, and 3 warps per scheduler.  This kernel
+//   * owns a 32 x TY tile per CTA (warp <-> row, lane <-> cell) and marches along z; the one-cell ring
+//     around the tile is handled by THREE extra warps (bottom row, top row, left+right columns) that
+//     run only the part of the scheme the tile needs from them (slopes, predictor, one predicted face
+//     state, at most one Riemann solve);
+//   * exchanges every neighbour quantity through shared memory: limited-slope neighbours are read from
+//     the staged primitive plane, the predicted "+" face state of a cell is written to the cell's own
+//     exchange slot, the neighbour on the other side of that face reads it, solves the Riemann problem
+//     once and writes the flux back INTO THE SAME SLOT, where the first cell picks it up as the flux
+//     through its upper face;
+//   * stages planes (tile + 2 ghost layers, all fields) with one TMA bulk-tensor copy each into a
+//     3-deep ring, so a plane has a whole iteration to arrive;
+//   * trims the arithmetic: reciprocal / square root = MUFU seed + one cubic correction, limiters on
+//     pre-scaled one-sided differences, flux differences accumulated straight into the half-step
+//     increment, tangential momentum and scalar fluxes as (value x mass flux);
+//   * keeps geometry out of registers on bitwise-uniform Cartesian grids (UNI: kernel-parameter
+//     constants), and as per-thread / per-plane 1-D table products otherwise.
+//
+// PAPER.md: Eq. 17 (slopes), Eq. 18 + Toro 16.5 (unsplit predictor), Eq. 19 (update), L201 (HLL/HLLC),
+// Eq. 13-16 (spherical sources), Eq. 2-3 (gravity); readings R1-R25.
+#pragma once
+#include <cuda.h>
+
+#include "hx_common.cuh"
+
+namespace hx {
+namespace t2 {
+
+constexpr int TX = 32;        // owner cells per tile row = one warp
+constexpr int PX = TX + 4;    // staged plane row: tile + 2 ghost cells on each side (36 * 8 B = 18 * 16 B)
+constexpr int TY_DEFAULT = 13;
+
+enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2 };   // GRAV_Z: acceleration along direction 2 only
+
+struct Args {
+  StepArgs s;
+  int zc;            // planes per z chunk
+  // UNI instantiations only (bitwise-uniform Cartesian tables): constants of the three axes
+  double uf[3];      // hw * idx   (slope pre-scale, = 1/2 up to rounding)
+  double uhc[3];     // (dt/2) / delta_d
+  double uil[3];     // 1 / delta_d  (CFL inverse lengths)
+};
+
+template <int NV, int TY>
+struct Smem {
+  static constexpr int PY = TY + 4;
+  static constexpr int NF = NV + 2;
+  static constexpr int FSTR = PY * PX;                         // field stride inside a plane (doubles)
+  static constexpr size_t plane_bytes = (size_t)NV * FSTR * sizeof(double);
+  static constexpr size_t plane_stride = (plane_bytes + 127) / 128 * 128;
+  static constexpr int NPL = 3;
+  static constexpr int XP = TX + 2;                            // x-exchange row pitch: slots ex = -1 .. TX-1 (+1 pad)
+  static constexpr int XSTR = TY * XP;                         // field stride of the x-exchange buffer
+  static constexpr int YSTR = (TY + 1) * TX;                   // y-exchange: slots ey = -1 .. TY-1
+  static constexpr size_t x_bytes = (size_t)NF * XSTR * sizeof(double);
+  static constexpr size_t y_bytes = (size_t)NF * YSTR * sizeof(double);
+  static constexpr size_t total = NPL * plane_stride + x_bytes + y_bytes + 64 + 128;
+};
+
+// ------------------------------------------------------------------------------------------------
+// fp64 helpers.  rcp.approx / rsqrt.approx give ~20 good bits (the low input word is ignored); one
+// cubic correction brings the relative error to ~(2^-19)^3 = 2^-57, below one ulp.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rcp3(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y, 1.0);
+  const double t = fma(e, e, e);
+  return fma(y, t, y);
+}
+
+__device__ __forceinline__ double sqrt3(double x) {   // x > 0
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double t = x * y;                       // ~ sqrt(x) (1 + d)
+  const double e = fma(-t, y, 1.0);             // 1 - x y^2
+  const double q = fma(0.375, e, 0.5) * e;      // (1 - e)^(-1/2) - 1 = e/2 + 3 e^2/8 + O(e^3)
+  return fma(t, q, t);
+}
+
+__device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
+
+// limiter on one-sided differences a (backward), b (forward); all are homogeneous of degree 1
+template <int LIM>
+__device__ __forceinline__ double lim_core(int lim_rt, double a, double b) {
+  if (LIM == HX_LIM_MINMOD) {
+    const bool opp = (hi32(a) ^ hi32(b)) < 0;
+    const double r = (fabs(a) < fabs(b)) ? a : b;
+    return opp ? 0.0 : r;
+  }
+  if (LIM == HX_LIM_MC) {
+    const bool opp = (hi32(a) ^ hi32(b)) < 0;
+    const double c = 0.5 * (a + b);
+    const double m = (fabs(a) < fabs(b)) ? a : b;
+    const double m2 = m + m;
+    const double r = (fabs(m2) < fabs(c)) ? m2 : c;
+    return opp ? 0.0 : r;
+  }
+  return limited_slope(LIM < 0 ? lim_rt : LIM, a, b);
+}
+
+// hw * lim(dm * idx_lo, dp * idx_hi)  (Eq. 17 with R5); fl = hw*idx_lo, fh = hw*idx_hi
+template <int LIM, bool UNI>
+__device__ __forceinline__ double lim_pre(int lim_rt, double dm, double dp, double fl, double fh) {
+  if (LIM == HX_LIM_NONE) return 0.0;
+  if (UNI) return fl * lim_core<LIM>(lim_rt, dm, dp);
+  return lim_core<LIM>(lim_rt, dm * fl, dp * fh);
+}
+
+// ------------------------------------------------------------------------------------------------
+// TMA / mbarrier PTX
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "T2_WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra.uni T2_WAIT_DONE;\n"
+      "bra.uni T2_WAIT_LOOP;\n"
+      "T2_WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_plane(const CUtensorMap* tmap, void* dst, uint64_t* bar, int x, int y, int z) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+          smem_u32(dst)),
+      "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(0), "r"(smem_u32(bar))
+      : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// Pointwise pieces of the scheme.  Field order of W / U: rho, u|m [3], P|E, scalars f|rho f.
+// ------------------------------------------------------------------------------------------------
+template <int NV>
+__device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, double* W) {   // Eq. 1, Eq. 5
+  const double ir = rcp3(U[0]);
+  W[0] = U[0];
+  W[1] = U[1] * ir;
+  W[2] = U[2] * ir;
+  W[3] = U[3] * ir;
+  const double ke2 = fma(U[3], W[3], fma(U[2], W[2], U[1] * W[1]));
+  W[4] = P.gm1 * fma(-0.5, ke2, U[4]);
+#pragma unroll
+  for (int s = 5; s < NV; ++s) W[s] = U[s] * ir;
+}
+
+// One face of the cell along DIR: face primitives Wc + sgn t (Eq. 17), their conserved form Uf, and the
+// analytic flux of that state accumulated into the half-step increment dU with the signed, (dt/2)-scaled
+// area/volume coefficient `coef` (Eq. 18: + for the lower face, - for the upper face).
+template <int NV, int DIR, bool PLUS>
+__device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double coef, double* Uf, double* dU) {
+  double Wf[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) Wf[v] = PLUS ? (Wc[v] + t[v]) : (Wc[v] - t[v]);
+  const double r = Wf[0];
+  Uf[0] = r;
+  Uf[1] = r * Wf[1];
+  Uf[2] = r * Wf[2];
+  Uf[3] = r * Wf[3];
+  const double ke2 = fma(Uf[3], Wf[3], fma(Uf[2], Wf[2], Uf[1] * Wf[1]));
+  Uf[4] = fma(0.5, ke2, Wf[4] * P.igm1);
+  const double unc = Wf[1 + DIR] * coef;
+  dU[0] = fma(r, unc, dU[0]);
+  dU[1] = fma(Uf[1], unc, dU[1]);
+  dU[2] = fma(Uf[2], unc, dU[2]);
+  dU[3] = fma(Uf[3], unc, dU[3]);
+  dU[1 + DIR] = fma(Wf[4], coef, dU[1 + DIR]);
+  dU[4] = fma(Uf[4] + Wf[4], unc, dU[4]);
+#pragma unroll
+  for (int s = 5; s < NV; ++s) {
+    Uf[s] = r * Wf[s];
+    dU[s] = fma(Uf[s], unc, dU[s]);
+  }
+}
+
+// Predicted face state U^{n+1/2} = cons(Wf) + dU (Eq. 18) as the record the Riemann solver consumes:
+// q = rho, u[3], P, E, c_s, scalars f.
+template <int NV>
+__device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, const double* dU, double* q) {
+  const double r = Uf[0] + dU[0];
+  const double ir = rcp3(r);
+  const double m1 = Uf[1] + dU[1], m2 = Uf[2] + dU[2], m3 = Uf[3] + dU[3];
+  const double E = Uf[4] + dU[4];
+  const double u1 = m1 * ir, u2 = m2 * ir, u3 = m3 * ir;
+  const double ke2 = fma(m3, u3, fma(m2, u2, m1 * u1));
+  const double p = P.gm1 * fma(-0.5, ke2, E);
+  q[0] = r;
+  q[1] = u1;
+  q[2] = u2;
+  q[3] = u3;
+  q[4] = p;
+  q[5] = E;
+  q[6] = sqrt3(P.gamma * p * ir);
+#pragma unroll
+  for (int s = 5; s < NV; ++s) q[2 + s] = (Uf[s] + dU[s]) * ir;
+}
+
+// HLL / HLLC flux along DIR from two records (L | R): F = rho, m[3], E, scalars.  Davis wave speeds
+// (R14), ties per R15.  Tangential momenta and scalars ride the mass flux: F_K + S_K (U*_K - U_K)
+// = q_K (rho_K u_K + S_K (rho*_K - rho_K)) for every quantity advected with the contact.
+template <int NV, int RS, int DIR>
+__device__ __forceinline__ void riemann_fs(const Phys& P, const double* L, const double* R, double* F) {
+  constexpr int NF = NV + 2;
+  const double uL = L[1 + DIR], uR = R[1 + DIR];
+  const double SL = fmin(uL - L[6], uR - R[6]);
+  const double SR = fmax(uL + L[6], uR + R[6]);
+  const bool hllc = (RS == HX_RIEMANN_HLLC) || (RS < 0 && P.riemann == HX_RIEMANN_HLLC);
+  if (hllc) {
+    const double dL = SL - uL, dR = SR - uR;
+    const double mL = L[0] * dL, mR = R[0] * dR;
+    const double Ss = (R[4] - L[4] + uL * mL - uR * mR) * rcp3(mL - mR);
+    const bool left = (SL >= 0.0) || (Ss >= 0.0);
+    const bool upwind = (SL >= 0.0) || (!left && SR <= 0.0);   // pure F_L or F_R
+    double qk[NF];
+#pragma unroll
+    for (int v = 0; v < NF; ++v) qk[v] = left ? L[v] : R[v];
+    const double SK = left ? SL : SR, mK = left ? mL : mR, dK = left ? dL : dR;
+    const double rK = qk[0], uK = qk[1 + DIR], pK = qk[4], EK = qk[5];
+    const double w = rcp3(SK - Ss);
+    const double fac = mK * w;                      // rho*_K
+    const double fr = rK * uK;                      // mass flux of side K
+    const double SKe = upwind ? 0.0 : SK;
+    const double F0 = fma(SKe, fac - rK, fr);
+    F[0] = F0;
+    F[1] = F0 * qk[1];
+    F[2] = F0 * qk[2];
+    F[3] = F0 * qk[3];
+    F[1 + DIR] = fma(SKe, fma(fac, Ss, -fr), fma(fr, uK, pK));   // normal: F_K + S_K (rho* S* - rho_K u_K)
+    const double Es = fma(dK * w, EK, (Ss - uK) * fma(fac, Ss, pK * w));   // E*_K
+    F[4] = fma(SKe, Es - EK, (EK + pK) * uK);
+#pragma unroll
+    for (int s = 5; s < NV; ++s) F[s] = F0 * qk[2 + s];
+  } else {
+    // HLL: (SR F_L - SL F_R + SL SR (U_R - U_L)) / (SR - SL), upwind flux outside the fan
+    const bool useL = SL >= 0.0, useR = (!useL) && SR <= 0.0;
+    const double iw = rcp3(SR - SL);
+    const double aL = useL ? 1.0 : (useR ? 0.0 : SR * iw), aR = useL ? 0.0 : (useR ? 1.0 : -SL * iw);
+    const double dd = (useL || useR) ? 0.0 : SL * SR * iw;
+    const double frL = L[0] * uL, frR = R[0] * uR;
+    F[0] = aL * frL + aR * frR + dd * (R[0] - L[0]);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double mL = L[0] * L[1 + d], mR = R[0] * R[1 + d];
+      const double fL = mL * uL + (d == DIR ? L[4] : 0.0), fR = mR * uR + (d == DIR ? R[4] : 0.0);
+      F[1 + d] = aL * fL + aR * fR + dd * (mR - mL);
+    }
+    F[4] = aL * ((L[5] + L[4]) * uL) + aR * ((R[5] + R[4]) * uR) + dd * (R[5] - L[5]);
+#pragma unroll
+    for (int s = 5; s < NV; ++s) {
+      const double sL = L[0] * L[2 + s], sR = R[0] * R[2 + s];
+      F[s] = aL * (sL * uL) + aR * (sR * uR) + dd * (sR - sL);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// The kernel.  Thread roles (warp-uniform except in the last warp):
+//   warps 0..TY-1  owners of row ey = warp, cell ex = lane
+//   warp  TY       bottom ring row  ey = -1   -> provides the predicted y+ state of its cells
+//   warp  TY+1     top ring row     ey = TY   -> solves the y face below it
+//   warp  TY+2     lanes 0..15 left ring column ex = -1 (x+ state), lanes 16..31 right ring column ex = TX (x face)
+// ------------------------------------------------------------------------------------------------
+template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int TY>
+__global__ void __launch_bounds__((TY + 3) * 32, 1)
+step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Args a) {
+  static_assert(TY >= 1 && TY <= 16, "the side-ring warp holds two columns of at most 16 cells");
+  static_assert(!(UNI && SPH), "UNI is for Cartesian grids");
+  using SM = Smem<NV, TY>;
+  constexpr int NF = SM::NF, FSTR = SM::FSTR, XSTR = SM::XSTR, YSTR = SM::YSTR, XP = SM::XP;
+  constexpr int PSTR = (int)(SM::plane_stride / sizeof(double));
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* base = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  double* planes = (double*)base;
+  double* X = (double*)(base + SM::NPL * SM::plane_stride);
+  double* Y = X + NF * XSTR;
+  uint64_t* mbar = (uint64_t*)(Y + NF * YSTR);
+
+  const StepArgs& s = a.s;
+  const Layout& L = s.L;
+  const Tables& T = s.T;
+  const Phys& P = s.P;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const bool owner = wid < TY;
+  int ex, ey, xoff = 0, coff = 0;     // tile coordinates; extra cells this thread converts (offsets from its own)
+  bool act = true;
+  if (owner) {
+    ex = lane;
+    ey = wid;
+  } else if (wid == TY) {
+    ex = lane;
+    ey = -1;
+    xoff = -PX;
+    coff = (lane == 0) ? -1 : (lane == 31 ? 1 : 0);
+  } else if (wid == TY + 1) {
+    ex = lane;
+    ey = TY;
+    xoff = PX;
+    coff = (lane == 0) ? -1 : (lane == 31 ? 1 : 0);
+  } else {
+    const int l = lane & 15;
+    ex = (lane >> 4) ? TX : -1;
+    ey = min(l, TY - 1);
+    act = l < TY;
+    xoff = (lane >> 4) ? 1 : -1;
+  }
+  const bool wr_px = (owner || (wid == TY + 2 && ex < 0)) && act;      // writes its predicted x+ state
+  const bool do_rx = (owner || (wid == TY + 2 && ex >= TX)) && act;    // solves the x face on its lower side
+  const bool wr_py = owner || wid == TY;
+  const bool do_ry = owner || wid == TY + 1;
+
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const int k0 = blockIdx.z * a.zc, k1 = min(L.n[2], k0 + a.zc);
+  const int i = i0 + ex, j = j0 + ey;                       // interior indices of this thread's column
+  const bool st_ok = owner && i < L.n[0] && j < L.n[1];
+  const int cidx = (ey + 2) * PX + (ex + 2);                // offset of the own cell inside one field of a plane
+  const int xs_own = ey * XP + ex + 1, xs_nbr = ey * XP + ex;
+  const int ys_own = (ey + 1) * TX + ex, ys_nbr = ey * TX + ex;
+  const bool lim_none = (LIM == HX_LIM_NONE) || (LIM < 0 && P.limiter == HX_LIM_NONE);   // R19: no predictor
+
+  // ---- loop-invariant geometry of this column, (dt/2) folded in -----------------------------------
+  const double hdt = 0.5 * s.dt;
+  const int pi = min(max(i + NG, 1), L.np[0] - 2), pj = min(max(j + NG, 1), L.np[1] - 2);
+  double flx, fhx, fly, fhy, hcm0, hcp0, hcm1, hcp1, c2m, c2p, il0, il1, il2xy;
+  if (UNI) {
+    flx = fhx = a.uf[0];
+    fly = fhy = a.uf[1];
+    hcm0 = hcp0 = a.uhc[0];
+    hcm1 = hcp1 = a.uhc[1];
+    c2m = c2p = a.uhc[2];
+    il0 = a.uil[0];
+    il1 = a.uil[1];
+    il2xy = a.uil[2];
+  } else {
+    const double hwx = T.hw[0][pi], hwy = T.hw[1][pj];
+    flx = hwx * T.idx[0][pi];
+    fhx = hwx * T.idx[0][pi + 1];
+    fly = hwy * T.idx[1][pj];
+    fhy = hwy * T.idx[1][pj + 1];
+    hcm0 = hdt * (T.cf[0][0][0][pi] * T.cf[0][0][1][pj]);
+    hcp0 = hdt * (T.cf[0][1][0][pi] * T.cf[0][1][1][pj]);
+    hcm1 = hdt * (T.cf[1][0][0][pi] * T.cf[1][0][1][pj]);
+    hcp1 = hdt * (T.cf[1][1][0][pi] * T.cf[1][1][1][pj]);
+    c2m = hdt * (T.cf[2][0][0][pi] * T.cf[2][0][1][pj]);
+    c2p = hdt * (T.cf[2][1][0][pi] * T.cf[2][1][1][pj]);
+    il0 = T.lf[0][0][pi] * T.lf[0][1][pj];
+    il1 = T.lf[1][0][pi] * T.lf[1][1][pj];
+    il2xy = T.lf[2][0][pi] * T.lf[2][1][pj];
+  }
+  // update coefficients dt dS/dV of the x and y faces; in spherical geometry the angular components
+  // carry the (1 -+ rr), (1 -+ st) factors of Eq. 14 (angular-momentum conserving form)
+  const double k0m = 2.0 * hcm0, k0p = 2.0 * hcp0, k1m = 2.0 * hcm1, k1p = 2.0 * hcp1;
+  double kxm = k0m, kxp = k0p, kym = k1m, kyp = k1p, hgr = 0.0, hAr = 0.0, hcgt = 0.0, hcAt = 0.0;
+  if (SPH) {
+    const double rr = T.rr[pi], st = T.st[pj], crg = T.cr[pi];
+    kxm = k0m * (1.0 - rr);
+    kxp = k0p * (1.0 + rr);
+    kym = k1m * (1.0 - st);
+    kyp = k1p * (1.0 + st);
+    hgr = hdt * T.gr[pi];
+    hAr = hdt * T.Ar[pi];
+    hcgt = hdt * crg * T.gt[pj];
+    hcAt = hdt * crg * T.At[pj];
+  }
+  const double hgx = (GRAV == GRAV_ANY) ? hdt * T.grav[0][pi] : 0.0;
+  const double hgy = (GRAV == GRAV_ANY) ? hdt * T.grav[1][pj] : 0.0;
+
+  // ---- TMA prologue: planes k0-2, k0-1, k0 -------------------------------------------------------------
+  const int xs = i0 + L.lead, ys = j0;                      // box origin in storage coordinates (cell i0-2, j0-2)
+  uint32_t phase = 0u;
+  if (threadIdx.x == 0) {
+    mbar_init(&mbar[0], 1);
+    mbar_init(&mbar[1], 1);
+    mbar_init(&mbar[2], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+      mbar_expect_tx(&mbar[b], (uint32_t)SM::plane_bytes);
+      tma_load_plane(&tmap, planes + b * PSTR, &mbar[b], xs, ys, k0 - 2 + b + NG);
+    }
+  }
+
+  // raw conserved -> primitive of the cell at offset `off` of plane `pl`, in place if `store`
+  auto convert = [&](double* pl, int off, double* Wout, bool store) {
+    double U[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) U[v] = pl[v * FSTR + off];
+    prim_of_cons<NV>(P, U, Wout);
+    if (store) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) pl[v * FSTR + off] = Wout[v];
+    }
+  };
+  // own cell + the ghost cells this thread is responsible for (every needed cell of the box exactly once)
+  auto convert_plane = [&](double* pl, double* Wown) {
+    convert(pl, cidx, Wown, act);
+    if (xoff != 0 && act) {
+      double tmp[NV];
+      convert(pl, cidx + xoff, tmp, true);
+      if (coff != 0) convert(pl, cidx + coff, tmp, true);
+    }
+  };
+
+  double dzm[NV];             // W(p) - W(p-1) of this column
+  {
+    double Wm2[NV], Wc0[NV];
+    mbar_wait(&mbar[0], 0u);
+    convert(planes, cidx, Wm2, false);
+    mbar_wait(&mbar[1], 0u);
+    phase = 3u;
+    convert_plane(planes + PSTR, Wc0);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) dzm[v] = Wc0[v] - Wm2[v];
+    __syncthreads();          // everyone has read plane k0-2: its buffer takes plane k0+1
+    if (threadIdx.x == 0) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(&mbar[0], (uint32_t)SM::plane_bytes);
+      tma_load_plane(&tmap, planes, &mbar[0], xs, ys, k0 + 1 + NG);
+    }
+  }
+
+  double zp[NF];              // predicted state on the upper z face of the previous plane
+  double Up[NV];              // partially updated cell of the previous plane
+  double Un0 = 0.0, Unm[3] = {0.0, 0.0, 0.0};   // rho^n, m^n of the previous plane (time-centred gravity)
+  double rate_max = 0.0;
+  bool bad = false;
+#pragma unroll
+  for (int v = 0; v < NF; ++v) zp[v] = 1.0;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) Up[v] = 1.0;
+  double* outp = s.Uout + L.off(min(i, L.n[0] - 1) + NG, min(j, L.n[1] - 1) + NG, k0 - 2 + NG);   // cell (i, j, p-1) at p = k0-1
+
+  int bc = 1;                 // buffer of plane p
+  for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
+    const int pk = p + NG;
+    const int bn = (bc == 2) ? 0 : bc + 1;
+    const bool do_xy = (p >= k0) && (p < k1);
+    double* Pc = planes + bc * PSTR;
+    double* Pn = planes + bn * PSTR;
+
+    // ---- [A] plane p+1 arrives: cons -> prim in place ---------------------------------------------
+    double Wn[NV];
+    mbar_wait(&mbar[bn], (phase >> bn) & 1u);
+    phase ^= (1u << bn);
+    convert_plane(Pn, Wn);
+
+    // per-plane z geometry (uniform addresses)
+    double flz, fhz, hcm2, hcp2;
+    if (UNI) {
+      flz = fhz = a.uf[2];
+      hcm2 = hcp2 = a.uhc[2];
+    } else {
+      const double hwz = __ldg(T.hw[2] + pk);
+      flz = hwz * __ldg(T.idx[2] + pk);
+      fhz = hwz * __ldg(T.idx[2] + pk + 1);
+      hcm2 = c2m * __ldg(T.cf[2][0][2] + pk);
+      hcp2 = c2p * __ldg(T.cf[2][1][2] + pk);
+    }
+    const double hgz = (GRAV != GRAV_OFF) ? hdt * __ldg(T.grav[2] + pk) : 0.0;
+
+    // ---- [B] O2-O4: limited slopes, face states, half-step increment dU (Eq. 17-18, unsplit) ---------
+    double Wc[NV], dU[NV];
+    double Uxm[NV], Uxp[NV], Uym[NV], Uyp[NV], Uzm[NV], Uzp[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      Wc[v] = Pc[v * FSTR + cidx];
+      dU[v] = 0.0;
+    }
+    {
+      double t[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const double dp = Wn[v] - Wc[v];
+        t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
+        dzm[v] = dp;
+      }
+      face_cons_flux<NV, 2, false>(P, Wc, t, hcm2, Uzm, dU);
+      face_cons_flux<NV, 2, true>(P, Wc, t, -hcp2, Uzp, dU);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
+        t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
+      }
+      face_cons_flux<NV, 0, false>(P, Wc, t, hcm0, Uxm, dU);
+      face_cons_flux<NV, 0, true>(P, Wc, t, -hcp0, Uxp, dU);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
+        t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
+      }
+      face_cons_flux<NV, 1, false>(P, Wc, t, hcm1, Uym, dU);
+      face_cons_flux<NV, 1, true>(P, Wc, t, -hcp1, Uyp, dU);
+    }
+    const double rho = Wc[0];
+    const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
+    if (SPH) {   // cell-centred geometric sources (R8)
+      const double ur = Wc[1], ut = Wc[2], up = Wc[3], pr = Wc[4];
+      dU[1] = fma(fma(mcy, ut, fma(mcz, up, 2.0 * pr)), hgr, dU[1]);
+      dU[2] += fma(mcz, up, pr) * hcgt - mcy * ur * hAr;
+      dU[3] -= mcz * fma(ur, hAr, ut * hcAt);
+    }
+    if (GRAV == GRAV_ANY) {
+      dU[1] = fma(rho, hgx, dU[1]);
+      dU[2] = fma(rho, hgy, dU[2]);
+      dU[4] = fma(mcx, hgx, fma(mcy, hgy, dU[4]));
+    }
+    if (GRAV != GRAV_OFF) {
+      dU[3] = fma(rho, hgz, dU[3]);
+      dU[4] = fma(mcz, hgz, dU[4]);
+    }
+    if (lim_none) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) dU[v] = 0.0;
+    }
+
+    // ---- [C] z direction, owners only: face p-1/2, finish cell p-1, start cell p ---------------------
+    if (owner) {
+      double Fz[NV];
+      if (p >= k0) {
+        double fzm[NF];
+        pred_state<NV>(P, Uzm, dU, fzm);
+        riemann_fs<NV, RS, 2>(P, zp, fzm, Fz);
+      }
+      if (p > k0) {   // the flux through the upper z face of cell p-1 is Fz: write the cell once
+        const double k2p = 2.0 * (UNI ? a.uhc[2] : c2p * __ldg(T.cf[2][1][2] + pk - 1));
+        double Unew[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Unew[v] = fma(-k2p, Fz[v], Up[v]);
+        if (SPH) {   // upper phi-face half of F^phi_phi in S_r and S_theta (Eq. 16 as read in R10, R11)
+          Unew[1] = fma(hgr, Fz[3], Unew[1]);
+          Unew[2] = fma(hcgt, Fz[3], Unew[2]);
+        }
+        if (GRAV != GRAV_OFF) {   // time-centred (R13)
+          const double hgzp = hdt * __ldg(T.grav[2] + pk - 1);
+          const double rs = Un0 + Unew[0];
+          if (GRAV == GRAV_ANY) {
+            const double m1 = fma(rs, hgx, Unew[1]), m2 = fma(rs, hgy, Unew[2]);
+            Unew[4] = fma(Unm[0] + m1, hgx, fma(Unm[1] + m2, hgy, Unew[4]));
+            Unew[1] = m1;
+            Unew[2] = m2;
+          }
+          const double m3 = fma(rs, hgzp, Unew[3]);
+          Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
+          Unew[3] = m3;
+        }
+        // A7: CFL rate of the new state + positivity check
+        const double ir = rcp3(Unew[0]);
+        const double u1 = Unew[1] * ir, u2 = Unew[2] * ir, u3 = Unew[3] * ir;
+        const double ke2 = fma(Unew[3], u3, fma(Unew[2], u2, Unew[1] * u1));
+        const double pn = P.gm1 * fma(-0.5, ke2, Unew[4]);
+        const double cs = sqrt3(P.gamma * pn * ir);
+        const double il2 = UNI ? a.uil[2] : il2xy * __ldg(T.lf[2][2] + pk - 1);
+        const double rate = fma(fabs(u1) + cs, il0, fma(fabs(u2) + cs, il1, (fabs(u3) + cs) * il2));
+        if (st_ok) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) outp[v * L.sv] = Unew[v];
+          // pn <= 0 or rho, pn of opposite sign make cs (hence rate) NaN; both negative is caught by rho > 0
+          if ((Unew[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL))) rate_max = fmax(rate_max, rate);
+          else bad = true;
+        }
+      }
+      if (do_xy) {   // U^n of cell p + the lower z face
+        double Un[NV];
+        Un[0] = rho;
+        Un[1] = mcx;
+        Un[2] = mcy;
+        Un[3] = mcz;
+        Un[4] = fma(0.5, fma(mcz, Wc[3], fma(mcy, Wc[2], mcx * Wc[1])), Wc[4] * P.igm1);
+#pragma unroll
+        for (int v = 5; v < NV; ++v) Un[v] = rho * Wc[v];
+        const double k2m = 2.0 * hcm2;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Up[v] = fma(k2m, Fz[v], Un[v]);
+        if (SPH) {
+          Up[1] = fma(hgr, Fz[3], Up[1]);
+          Up[2] = fma(hcgt, Fz[3], Up[2]);
+        }
+        if (GRAV != GRAV_OFF) {
+          Un0 = rho;
+          Unm[0] = mcx;
+          Unm[1] = mcy;
+          Unm[2] = mcz;
+        }
+      }
+      if (p < k1) pred_state<NV>(P, Uzp, dU, zp);
+    }
+
+    // ---- [D] predicted "+" states of the x and y faces go to the exchange slots ------------------------
+    if (do_xy) {
+      if (wr_px) {
+        double q[NF];
+        pred_state<NV>(P, Uxp, dU, q);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
+      }
+      if (wr_py) {
+        double q[NF];
+        pred_state<NV>(P, Uyp, dU, q);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
+      }
+    }
+    __syncthreads();                                   // (1) "+" states visible; all reads of plane p done
+    if (threadIdx.x == 0 && p + 3 <= k1 + 1) {         // plane p+3 takes the buffer of plane p
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(&mbar[bc], (uint32_t)SM::plane_bytes);
+      tma_load_plane(&tmap, Pc, &mbar[bc], xs, ys, p + 3 + NG);
+    }
+
+    // ---- [E] x and y faces on the lower side of this cell: Riemann flux once, back into the slot -----
+    if (do_xy) {
+      if (do_rx) {
+        double ql[NF], qr[NF], F[NV];
+        pred_state<NV>(P, Uxm, dU, qr);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) ql[v] = X[v * XSTR + xs_nbr];
+        riemann_fs<NV, RS, 0>(P, ql, qr, F);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) X[v * XSTR + xs_nbr] = F[v];
+        if (owner) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) Up[v] = fma((SPH && (v == 2 || v == 3)) ? kxm : k0m, F[v], Up[v]);
+        }
+      }
+      if (do_ry) {
+        double ql[NF], qr[NF], F[NV];
+        pred_state<NV>(P, Uym, dU, qr);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) ql[v] = Y[v * YSTR + ys_nbr];
+        riemann_fs<NV, RS, 1>(P, ql, qr, F);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
+        if (owner) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) Up[v] = fma((SPH && v == 3) ? kym : k1m, F[v], Up[v]);
+          if (SPH) Up[1] = fma(hgr, F[2], Up[1]);
+        }
+      }
+    }
+    __syncthreads();                                   // (2) fluxes visible
+    // ---- [F] fluxes through the upper x and y faces come back in the own slots -------------------------
+    if (do_xy && owner) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? kxp : k0p), X[v * XSTR + xs_own], Up[v]);
+      if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? kyp : k1p), Y[v * YSTR + ys_own], Up[v]);
+    }
+    bc = bn;
+  }
+
+  if (bad) atomicOr(s.status, 1);
+  block_rate_max(rate_max, s.rate_bits);
+}
+
+}  // namespace t2
+}  // namespace hx

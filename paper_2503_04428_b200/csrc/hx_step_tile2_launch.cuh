@@ -1,0 +1,45 @@
+// hx_step_tile2_launch.cuh -- launch dispatch of the fused step kernel for one field count NV.  Each
+// hx_step_tile2_nv<N>.cu instantiates launch_nv<N> so the variants compile in parallel.
+#pragma once
+#include "hx_step_tile2.cuh"
+
+namespace hx {
+namespace t2 {
+
+struct Plan {
+  CUtensorMap tmap[2];
+  int zc;
+  dim3 grid;
+  bool uni;          // bitwise-uniform Cartesian tables: geometry travels as kernel-parameter constants
+  bool grav_z;       // uniform gravity along direction 2 only
+  double uf[3], uiw[3];
+  const char* name;
+};
+
+template <int NV>
+cudaError_t launch_nv(Plan& plan, const Args& a, int cur, cudaStream_t st);
+
+template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI>
+static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  constexpr int TY = TY_DEFAULT;
+  auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Smem<NV, TY>::total);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  plan.name = UNI ? "tile2_uni" : "tile2";
+  kern<<<plan.grid, (TY + 3) * 32, Smem<NV, TY>::total, st>>>(plan.tmap[cur], a);
+  return cudaGetLastError();
+}
+
+// the runtime-switch build (limiter, solver, any gravity) covers every configuration of this NV
+template <int NV>
+static cudaError_t launch_generic(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.spherical) return launch_cfg<NV, true, GRAV_ANY, -1, -1, false>(plan, a, cur, st);
+  return launch_cfg<NV, false, GRAV_ANY, -1, -1, false>(plan, a, cur, st);
+}
+
+}  // namespace t2
+}  // namespace hx

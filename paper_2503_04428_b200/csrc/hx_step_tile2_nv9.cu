@@ -1,0 +1,14 @@
+// NV = 9 (3-D, four passive scalars).  Fully specialised: spherical wedge with point-mass gravity, minmod + HLLC
+// (config 5, wedge_3d).
+#include "hx_step_tile2_launch.cuh"
+namespace hx {
+namespace t2 {
+template <>
+cudaError_t launch_nv<9>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  const Phys& P = a.s.P;
+  if (P.spherical && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
+    return launch_cfg<9, true, GRAV_ANY, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);
+  return launch_generic<9>(plan, a, cur, st);
+}
+}  // namespace t2
+}  // namespace hx

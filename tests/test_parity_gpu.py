@@ -16,6 +16,7 @@ pytestmark = pytest.mark.gpu
 TOL_STEP = 1e-12
 TOL_L1 = 1e-9
 KERNELS = ["generic", "auto"]
+KERNELS_3D = KERNELS + ["tiled_v1"]     # the first tiled design stays selectable for A/B runs
 
 
 @pytest.fixture(scope="module")
@@ -31,6 +32,8 @@ def make_pair(hx, ox, spec, W, kernel="auto"):
     g = hx.Hydro(spec)
     if kernel == "generic":
         g.set_option(hx.OPT_KERNEL, hx.KERNEL_GENERIC)
+    elif kernel == "tiled_v1" and spec["ndim"] == 3:
+        g.set_option(hx.OPT_KERNEL, hx.KERNEL_TILED)
     g.set_state(np.ascontiguousarray(W), hx.PRIMITIVE)
     o = ox.Oracle(spec)
     o.set_state(W, ox.PRIMITIVE)
@@ -59,7 +62,7 @@ REDUCED = {
 }
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS_3D)
 @pytest.mark.parametrize("name", list(REDUCED))
 def test_one_step_parity(hx, oxlib, name, kernel):
     ox = oxlib
@@ -78,7 +81,7 @@ def test_one_step_parity(hx, oxlib, name, kernel):
     assert abs(dt_g2 - dt_o2) <= 1e-12 * dt_o2
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("kernel", KERNELS_3D)
 @pytest.mark.parametrize("name", list(REDUCED))
 def test_hundred_step_parity(hx, oxlib, name, kernel):
     ox = oxlib
@@ -188,6 +191,18 @@ def test_nonphysical_state_is_reported_not_floored(hx):
     assert e.value.code == hx.ERR_NONPHYSICAL
 
 
+def test_nonphysical_state_in_the_fused_3d_kernel(hx):
+    spec, W = wl.smooth_periodic(3, [40, 20, 12], seed=5, n_scalars=0)
+    g = hx.Hydro(spec)
+    g.set_state(W, hx.PRIMITIVE)
+    g.step(g.compute_dt(0.5))
+    assert g.step_kernel.startswith("tile2") and g.compute_dt(0.5) > 0
+    g.step(80.0 * g.compute_dt(0.5))
+    with pytest.raises(hx.HxError) as e:
+        g.compute_dt(0.5)
+    assert e.value.code == hx.ERR_NONPHYSICAL
+
+
 def test_minimum_sizes_and_degenerate_shapes(hx, oxlib):
     ox = oxlib
     for ndim, n in ((1, [2]), (2, [2, 3]), (3, [2, 2, 2]), (3, [3, 2, 5]), (1, [33])):
@@ -199,11 +214,10 @@ def test_minimum_sizes_and_degenerate_shapes(hx, oxlib):
         assert max(max_rel_per_field(g.get_state(), o.get_state(), ndim)) <= TOL_STEP, n
 
 
-@pytest.mark.parametrize("n", [(58, 20, 18), (87, 12, 8), (31, 11, 5), (30, 10, 16), (61, 21, 33)])
-def test_tile_edges_and_odd_widths(hx, oxlib, n):
-    """Grid widths that give odd balanced tile widths (58 -> 2 x 29), exactly full tiles, and one
-    cell more than a full tile, in x and y; z chunk boundaries.  (An odd TMA start coordinate of the
-    fp64 box is illegal on sm_100a: the plan must round tile widths to even.)"""
+@pytest.mark.parametrize("n", [(58, 20, 18), (64, 26, 8), (65, 27, 5), (33, 14, 16), (32, 13, 33), (96, 39, 70), (2, 2, 2), (5, 3, 2)])
+def test_tile_edges(hx, oxlib, n):
+    """Grids that give exactly full 32 x 13 tiles, one cell more than a full tile in x and y, ragged tails,
+    single partial tiles, and z extents that split into several chunks."""
     ox = oxlib
     spec, W = wl.smooth_periodic(3, list(n), seed=n[0], n_scalars=0, limiter=wl.LIM_MC)
     g, o = make_pair(hx, ox, spec, W, "auto")
@@ -211,5 +225,29 @@ def test_tile_edges_and_odd_widths(hx, oxlib, n):
         dt = o.compute_dt(0.5)
         g.step(dt)
         o.step(dt)
-    assert g.step_kernel == "tiled3d"
+    assert g.step_kernel.startswith("tile2")
     assert max(max_rel_per_field(g.get_state(), o.get_state(), 3)) <= 2 * TOL_STEP, n
+
+
+UNIFORM = {   # 2^k cells on dyadic extents: bitwise-uniform tables -> the constant-geometry instantiations
+    "sedov_3d": lambda: wl.sedov_3d((64, 32, 32)),
+    "rt_3d": lambda: wl.rt_3d((32, 64, 64)),
+}
+
+
+@pytest.mark.parametrize("name", list(UNIFORM))
+def test_uniform_grid_instantiations(hx, oxlib, name):
+    ox = oxlib
+    spec, W = UNIFORM[name]()
+    g, o = make_pair(hx, ox, spec, W)
+    for s in range(40):
+        dt_g, dt_o = g.compute_dt(spec["cfl"]), o.compute_dt(spec["cfl"])
+        assert abs(dt_g - dt_o) <= 1e-10 * dt_o, (s, dt_g, dt_o)
+        g.step(dt_g)
+        o.step(dt_o)
+        if s == 0:
+            assert g.step_kernel == "tile2_uni"
+            rel = max_rel_per_field(g.get_state(), o.get_state(), 3)
+            assert max(rel) <= TOL_STEP, (name, rel)
+    l1 = l1_rel_per_field(g.get_state(), o.get_state(), 3)
+    assert max(l1) <= TOL_L1, (name, l1)
