@@ -32,7 +32,10 @@ namespace t2 {
 
 constexpr int TX = 32;        // owner cells per tile row = one warp
 constexpr int PX = TX + 4;    // staged plane row: tile + 2 ghost cells on each side (36 * 8 B = 18 * 16 B)
-constexpr int TY_DEFAULT = 13;
+#ifndef HX_T2_TY
+#define HX_T2_TY 8
+#endif
+constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows + 3 ring warps = 11 warps: two owner warps per scheduler, ring warps spread over three
 
 enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2 };   // GRAV_Z: acceleration along direction 2 only
 
@@ -320,8 +323,6 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   }
   const bool wr_px = (owner || (wid == TY + 2 && ex < 0)) && act;      // writes its predicted x+ state
   const bool do_rx = (owner || (wid == TY + 2 && ex >= TX)) && act;    // solves the x face on its lower side
-  const bool wr_py = owner || wid == TY;
-  const bool do_ry = owner || wid == TY + 1;
 
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
   const int k0 = blockIdx.z * a.zc, k1 = min(L.n[2], k0 + a.zc);
@@ -530,15 +531,31 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       for (int v = 0; v < NV; ++v) dU[v] = 0.0;
     }
 
-    // ---- [C] z direction, owners only: face p-1/2, finish cell p-1, start cell p ---------------------
     if (owner) {
+      // ======== owners: one straight-line block up to the first barrier, so that the six independent
+      // predicted states, the z Riemann problem and the finish of cell p-1 can be interleaved ==========
+      double qxm[NF], qym[NF];
+      {
+        double q[NF];
+        pred_state<NV>(P, Uxp, dU, q);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
+        pred_state<NV>(P, Uyp, dU, q);
+#pragma unroll
+        for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
+      }
+      pred_state<NV>(P, Uxm, dU, qxm);
+      pred_state<NV>(P, Uym, dU, qym);
+      // ---- [C] z direction: face p-1/2, finish cell p-1, start cell p (edge iterations compute on valid
+      // but unused data; only the stores and the rate are predicated) -----------------------------------
       double Fz[NV];
-      if (p >= k0) {
+      {
         double fzm[NF];
         pred_state<NV>(P, Uzm, dU, fzm);
         riemann_fs<NV, RS, 2>(P, zp, fzm, Fz);
       }
-      if (p > k0) {   // the flux through the upper z face of cell p-1 is Fz: write the cell once
+      pred_state<NV>(P, Uzp, dU, zp);
+      {
         const double k2p = 2.0 * (UNI ? a.uhc[2] : c2p * __ldg(T.cf[2][1][2] + pk - 1));
         double Unew[NV];
 #pragma unroll
@@ -560,7 +577,13 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
           Unew[3] = m3;
         }
-        // A7: CFL rate of the new state + positivity check
+        const bool st = st_ok && (p > k0);
+        if (st) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) outp[v * L.sv] = Unew[v];
+        }
+        // A7: CFL rate of the new state + positivity check.  pn <= 0, or rho and pn of opposite sign, make cs
+        // (hence rate) NaN; both negative is caught by rho > 0.
         const double ir = rcp3(Unew[0]);
         const double u1 = Unew[1] * ir, u2 = Unew[2] * ir, u3 = Unew[3] * ir;
         const double ke2 = fma(Unew[3], u3, fma(Unew[2], u2, Unew[1] * u1));
@@ -568,15 +591,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         const double cs = sqrt3(P.gamma * pn * ir);
         const double il2 = UNI ? a.uil[2] : il2xy * __ldg(T.lf[2][2] + pk - 1);
         const double rate = fma(fabs(u1) + cs, il0, fma(fabs(u2) + cs, il1, (fabs(u3) + cs) * il2));
-        if (st_ok) {
-#pragma unroll
-          for (int v = 0; v < NV; ++v) outp[v * L.sv] = Unew[v];
-          // pn <= 0 or rho, pn of opposite sign make cs (hence rate) NaN; both negative is caught by rho > 0
-          if ((Unew[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL))) rate_max = fmax(rate_max, rate);
-          else bad = true;
-        }
+        const bool fine = (Unew[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL));
+        rate_max = (st && fine) ? fmax(rate_max, rate) : rate_max;
+        bad = bad || (st && !fine);
       }
-      if (do_xy) {   // U^n of cell p + the lower z face
+      {   // U^n of cell p + the lower z face
         double Un[NV];
         Un[0] = rho;
         Un[1] = mcx;
@@ -599,69 +618,81 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Unm[2] = mcz;
         }
       }
-      if (p < k1) pred_state<NV>(P, Uzp, dU, zp);
-    }
-
-    // ---- [D] predicted "+" states of the x and y faces go to the exchange slots ------------------------
-    if (do_xy) {
-      if (wr_px) {
-        double q[NF];
-        pred_state<NV>(P, Uxp, dU, q);
-#pragma unroll
-        for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
+      asm volatile("bar.sync 0;" ::: "memory");          // (1) "+" states visible; all reads of plane p done
+      if (threadIdx.x == 0 && p + 3 <= k1 + 1) {         // plane p+3 takes the buffer of plane p
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(&mbar[bc], (uint32_t)SM::plane_bytes);
+        tma_load_plane(&tmap, Pc, &mbar[bc], xs, ys, p + 3 + NG);
       }
-      if (wr_py) {
-        double q[NF];
+      // ---- [E] x and y faces on the lower side of this cell: Riemann flux once, back into the slot -----
+      if (do_xy) {
+        double qlx[NF], qly[NF], Fx[NV], Fy[NV];
+#pragma unroll
+        for (int v = 0; v < NF; ++v) {
+          qlx[v] = X[v * XSTR + xs_nbr];
+          qly[v] = Y[v * YSTR + ys_nbr];
+        }
+        riemann_fs<NV, RS, 0>(P, qlx, qxm, Fx);
+        riemann_fs<NV, RS, 1>(P, qly, qym, Fy);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          X[v * XSTR + xs_nbr] = Fx[v];
+          Y[v * YSTR + ys_nbr] = Fy[v];
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          Up[v] = fma((SPH && (v == 2 || v == 3)) ? kxm : k0m, Fx[v], Up[v]);
+          Up[v] = fma((SPH && v == 3) ? kym : k1m, Fy[v], Up[v]);
+        }
+        if (SPH) Up[1] = fma(hgr, Fy[2], Up[1]);
+      }
+      asm volatile("bar.sync 0;" ::: "memory");          // (2) fluxes visible
+      // ---- [F] fluxes through the upper x and y faces come back in the own slots -----------------------
+      if (do_xy) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? kxp : k0p), X[v * XSTR + xs_own], Up[v]);
+        if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? kyp : k1p), Y[v * YSTR + ys_own], Up[v]);
+      }
+    } else {
+      // ======== ring warps: one predicted state, at most one Riemann solve ================================
+      double q[NF];
+      if (wid == TY) {
         pred_state<NV>(P, Uyp, dU, q);
 #pragma unroll
         for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
-      }
-    }
-    __syncthreads();                                   // (1) "+" states visible; all reads of plane p done
-    if (threadIdx.x == 0 && p + 3 <= k1 + 1) {         // plane p+3 takes the buffer of plane p
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(&mbar[bc], (uint32_t)SM::plane_bytes);
-      tma_load_plane(&tmap, Pc, &mbar[bc], xs, ys, p + 3 + NG);
-    }
-
-    // ---- [E] x and y faces on the lower side of this cell: Riemann flux once, back into the slot -----
-    if (do_xy) {
-      if (do_rx) {
-        double ql[NF], qr[NF], F[NV];
-        pred_state<NV>(P, Uxm, dU, qr);
+      } else if (wid == TY + 1) {
+        pred_state<NV>(P, Uym, dU, q);
+      } else {
+        double Us[NV];
 #pragma unroll
-        for (int v = 0; v < NF; ++v) ql[v] = X[v * XSTR + xs_nbr];
-        riemann_fs<NV, RS, 0>(P, ql, qr, F);
+        for (int v = 0; v < NV; ++v) Us[v] = (ex < 0) ? Uxp[v] : Uxm[v];
+        pred_state<NV>(P, Us, dU, q);
+        if (wr_px) {
 #pragma unroll
-        for (int v = 0; v < NV; ++v) X[v * XSTR + xs_nbr] = F[v];
-        if (owner) {
-#pragma unroll
-          for (int v = 0; v < NV; ++v) Up[v] = fma((SPH && (v == 2 || v == 3)) ? kxm : k0m, F[v], Up[v]);
+          for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
         }
       }
-      if (do_ry) {
-        double ql[NF], qr[NF], F[NV];
-        pred_state<NV>(P, Uym, dU, qr);
+      asm volatile("bar.sync 0;" ::: "memory");          // (1)
+      if (do_xy) {
+        if (wid == TY + 1) {
+          double ql[NF], F[NV];
 #pragma unroll
-        for (int v = 0; v < NF; ++v) ql[v] = Y[v * YSTR + ys_nbr];
-        riemann_fs<NV, RS, 1>(P, ql, qr, F);
+          for (int v = 0; v < NF; ++v) ql[v] = Y[v * YSTR + ys_nbr];
+          riemann_fs<NV, RS, 1>(P, ql, q, F);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
-        if (owner) {
+          for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
+        } else if (do_rx) {
+          double ql[NF], F[NV];
 #pragma unroll
-          for (int v = 0; v < NV; ++v) Up[v] = fma((SPH && v == 3) ? kym : k1m, F[v], Up[v]);
-          if (SPH) Up[1] = fma(hgr, F[2], Up[1]);
+          for (int v = 0; v < NF; ++v) ql[v] = X[v * XSTR + xs_nbr];
+          riemann_fs<NV, RS, 0>(P, ql, q, F);
+#pragma unroll
+          for (int v = 0; v < NV; ++v) X[v * XSTR + xs_nbr] = F[v];
         }
       }
-    }
-    __syncthreads();                                   // (2) fluxes visible
-    // ---- [F] fluxes through the upper x and y faces come back in the own slots -------------------------
-    if (do_xy && owner) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? kxp : k0p), X[v * XSTR + xs_own], Up[v]);
-      if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
-#pragma unroll
-      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? kyp : k1p), Y[v * YSTR + ys_own], Up[v]);
+      asm volatile("bar.sync 0;" ::: "memory");          // (2)
     }
     bc = bn;
   }
