@@ -196,19 +196,18 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
 template <int NV>
 __device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, const double* dU, double* q) {
   const double r = Uf[0] + dU[0];
-  const double ir = rcp3(r);
   const double m1 = Uf[1] + dU[1], m2 = Uf[2] + dU[2], m3 = Uf[3] + dU[3];
   const double E = Uf[4] + dU[4];
-  const double u1 = m1 * ir, u2 = m2 * ir, u3 = m3 * ir;
-  const double ke2 = fma(m3, u3, fma(m2, u2, m1 * u1));
-  const double p = P.gm1 * fma(-0.5, ke2, E);
+  const double mm = fma(m3, m3, fma(m2, m2, m1 * m1));   // independent of 1/rho: shortens the dependent chain
+  const double ir = rcp3(r);
+  const double e = fma(-0.5 * ir, mm, E);                // internal energy density
   q[0] = r;
-  q[1] = u1;
-  q[2] = u2;
-  q[3] = u3;
-  q[4] = p;
+  q[1] = m1 * ir;
+  q[2] = m2 * ir;
+  q[3] = m3 * ir;
+  q[4] = P.gm1 * e;
   q[5] = E;
-  q[6] = sqrt3(P.gamma * p * ir);
+  q[6] = sqrt3((P.gamma * P.gm1) * ir * e);              // c^2 = gamma P / rho
 #pragma unroll
   for (int s = 5; s < NV; ++s) q[2 + s] = (Uf[s] + dU[s]) * ir;
 }
@@ -440,6 +439,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   double zp[NF];              // predicted state on the upper z face of the previous plane
   double Up[NV];              // partially updated cell of the previous plane
   double Un0 = 0.0, Unm[3] = {0.0, 0.0, 0.0};   // rho^n, m^n of the previous plane (time-centred gravity)
+  double Ul[5] = {1.0, 0.0, 0.0, 0.0, 1.0};     // rho, m, E of the cell written one iteration ago (deferred CFL rate)
+  bool st_l = false;                            // ... and whether it was stored
   double rate_max = 0.0;
   bool bad = false;
 #pragma unroll
@@ -448,22 +449,25 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   for (int v = 0; v < NV; ++v) Up[v] = 1.0;
   double* outp = s.Uout + L.off(min(i, L.n[0] - 1) + NG, min(j, L.n[1] - 1) + NG, k0 - 2 + NG);   // cell (i, j, p-1) at p = k0-1
 
-  int bc = 1;                 // buffer of plane p
-  for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
-    const int pk = p + NG;
-    const int bn = (bc == 2) ? 0 : bc + 1;
-    const bool do_xy = (p >= k0) && (p < k1);
-    double* Pc = planes + bc * PSTR;
-    double* Pn = planes + bn * PSTR;
+  // A7: CFL rate + positivity check of the cell in Ul (padded z index pkc).  e <= 0, or rho and e of opposite
+  // sign, make the sound speed (hence the rate) NaN; both negative is caught by rho > 0.  It runs one iteration
+  // after the cell was written so that its serial chain (1/rho -> e -> sqrt) overlaps the slope arithmetic.
+  auto cfl_rate = [&](int pkc) {
+    const double mm = fma(Ul[3], Ul[3], fma(Ul[2], Ul[2], Ul[1] * Ul[1]));
+    const double ir = rcp3(Ul[0]);
+    const double e = fma(-0.5 * ir, mm, Ul[4]);
+    const double cs = sqrt3((P.gamma * P.gm1) * ir * e);
+    const double il2 = UNI ? a.uil[2] : il2xy * __ldg(T.lf[2][2] + pkc);
+    const double rate = fma(fma(fabs(Ul[1]), ir, cs), il0, fma(fma(fabs(Ul[2]), ir, cs), il1, fma(fabs(Ul[3]), ir, cs) * il2));
+    const bool fine = (Ul[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL));
+    rate_max = (st_l && fine) ? fmax(rate_max, rate) : rate_max;
+    bad = bad || (st_l && !fine);
+  };
 
-    // ---- [A] plane p+1 arrives: cons -> prim in place ---------------------------------------------
-    double Wn[NV];
-    mbar_wait(&mbar[bn], (phase >> bn) & 1u);
-    phase ^= (1u << bn);
-    convert_plane(Pn, Wn);
-
-    // per-plane z geometry (uniform addresses)
-    double flz, fhz, hcm2, hcp2;
+  // [B] O2-O4 for the cell of plane p: limited slopes, face states, half-step increment dU (Eq. 17-18, unsplit)
+  auto predictor = [&](const double* Pc, const double* Wn, int pk, double* Wc, double* dU, double* Uxm, double* Uxp, double* Uym,
+                       double* Uyp, double* Uzm, double* Uzp, double& hcm2) {
+    double flz, fhz, hcp2;   // per-plane z geometry (uniform addresses)
     if (UNI) {
       flz = fhz = a.uf[2];
       hcm2 = hcp2 = a.uhc[2];
@@ -474,41 +478,34 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       hcm2 = c2m * __ldg(T.cf[2][0][2] + pk);
       hcp2 = c2p * __ldg(T.cf[2][1][2] + pk);
     }
-    const double hgz = (GRAV != GRAV_OFF) ? hdt * __ldg(T.grav[2] + pk) : 0.0;
-
-    // ---- [B] O2-O4: limited slopes, face states, half-step increment dU (Eq. 17-18, unsplit) ---------
-    double Wc[NV], dU[NV];
-    double Uxm[NV], Uxp[NV], Uym[NV], Uyp[NV], Uzm[NV], Uzp[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       Wc[v] = Pc[v * FSTR + cidx];
       dU[v] = 0.0;
     }
-    {
-      double t[NV];
+    double t[NV];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const double dp = Wn[v] - Wc[v];
-        t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
-        dzm[v] = dp;
-      }
-      face_cons_flux<NV, 2, false>(P, Wc, t, hcm2, Uzm, dU);
-      face_cons_flux<NV, 2, true>(P, Wc, t, -hcp2, Uzp, dU);
-#pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
-        t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
-      }
-      face_cons_flux<NV, 0, false>(P, Wc, t, hcm0, Uxm, dU);
-      face_cons_flux<NV, 0, true>(P, Wc, t, -hcp0, Uxp, dU);
-#pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
-        t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
-      }
-      face_cons_flux<NV, 1, false>(P, Wc, t, hcm1, Uym, dU);
-      face_cons_flux<NV, 1, true>(P, Wc, t, -hcp1, Uyp, dU);
+    for (int v = 0; v < NV; ++v) {
+      const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
+      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
     }
+    face_cons_flux<NV, 0, false>(P, Wc, t, hcm0, Uxm, dU);
+    face_cons_flux<NV, 0, true>(P, Wc, t, -hcp0, Uxp, dU);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
+      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
+    }
+    face_cons_flux<NV, 1, false>(P, Wc, t, hcm1, Uym, dU);
+    face_cons_flux<NV, 1, true>(P, Wc, t, -hcp1, Uyp, dU);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const double dp = Wn[v] - Wc[v];
+      t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
+      dzm[v] = dp;
+    }
+    face_cons_flux<NV, 2, false>(P, Wc, t, hcm2, Uzm, dU);
+    face_cons_flux<NV, 2, true>(P, Wc, t, -hcp2, Uzp, dU);
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
@@ -523,6 +520,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       dU[4] = fma(mcx, hgx, fma(mcy, hgy, dU[4]));
     }
     if (GRAV != GRAV_OFF) {
+      const double hgz = hdt * __ldg(T.grav[2] + pk);
       dU[3] = fma(rho, hgz, dU[3]);
       dU[4] = fma(mcz, hgz, dU[4]);
     }
@@ -530,10 +528,27 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
       for (int v = 0; v < NV; ++v) dU[v] = 0.0;
     }
+  };
 
+  int bc = 1;                 // buffer of plane p
+  for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
+    const int pk = p + NG;
+    const int bn = (bc == 2) ? 0 : bc + 1;
+    const bool do_xy = (p >= k0) && (p < k1);
+    double* Pc = planes + bc * PSTR;
+    double* Pn = planes + bn * PSTR;
+    mbar_wait(&mbar[bn], (phase >> bn) & 1u);            // plane p+1 has arrived (issued a whole iteration ago)
+    phase ^= (1u << bn);
+
+    double Wn[NV], Wc[NV], dU[NV], hcm2;
+    double Uxm[NV], Uxp[NV], Uym[NV], Uyp[NV], Uzm[NV], Uzp[NV];
     if (owner) {
-      // ======== owners: one straight-line block up to the first barrier, so that the six independent
-      // predicted states, the z Riemann problem and the finish of cell p-1 can be interleaved ==========
+      // ======== owners: ONE straight-line block up to the first barrier, so that the slope arithmetic, the six
+      // independent predicted states, the z Riemann problem, the finish of cell p-1 and the deferred CFL rate of
+      // cell p-2 can be interleaved by the scheduler ======================================================
+      cfl_rate(pk - 2);
+      convert(Pn, cidx, Wn, true);                       // [A] cons -> prim of the own cell of plane p+1, in place
+      predictor(Pc, Wn, pk, Wc, dU, Uxm, Uxp, Uym, Uyp, Uzm, Uzp, hcm2);
       double qxm[NF], qym[NF];
       {
         double q[NF];
@@ -547,7 +562,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       pred_state<NV>(P, Uxm, dU, qxm);
       pred_state<NV>(P, Uym, dU, qym);
       // ---- [C] z direction: face p-1/2, finish cell p-1, start cell p (edge iterations compute on valid
-      // but unused data; only the stores and the rate are predicated) -----------------------------------
+      // but unused data; only the store and the rate are predicated) ------------------------------------
       double Fz[NV];
       {
         double fzm[NF];
@@ -577,25 +592,17 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
           Unew[3] = m3;
         }
-        const bool st = st_ok && (p > k0);
-        if (st) {
+        st_l = st_ok && (p > k0);
+        if (st_l) {
 #pragma unroll
           for (int v = 0; v < NV; ++v) outp[v * L.sv] = Unew[v];
         }
-        // A7: CFL rate of the new state + positivity check.  pn <= 0, or rho and pn of opposite sign, make cs
-        // (hence rate) NaN; both negative is caught by rho > 0.
-        const double ir = rcp3(Unew[0]);
-        const double u1 = Unew[1] * ir, u2 = Unew[2] * ir, u3 = Unew[3] * ir;
-        const double ke2 = fma(Unew[3], u3, fma(Unew[2], u2, Unew[1] * u1));
-        const double pn = P.gm1 * fma(-0.5, ke2, Unew[4]);
-        const double cs = sqrt3(P.gamma * pn * ir);
-        const double il2 = UNI ? a.uil[2] : il2xy * __ldg(T.lf[2][2] + pk - 1);
-        const double rate = fma(fabs(u1) + cs, il0, fma(fabs(u2) + cs, il1, (fabs(u3) + cs) * il2));
-        const bool fine = (Unew[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL));
-        rate_max = (st && fine) ? fmax(rate_max, rate) : rate_max;
-        bad = bad || (st && !fine);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Ul[v] = Unew[v];
       }
       {   // U^n of cell p + the lower z face
+        const double rho = Wc[0];
+        const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
         double Un[NV];
         Un[0] = rho;
         Un[1] = mcx;
@@ -656,7 +663,9 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? kyp : k1p), Y[v * YSTR + ys_own], Up[v]);
       }
     } else {
-      // ======== ring warps: one predicted state, at most one Riemann solve ================================
+      // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
+      convert_plane(Pn, Wn);
+      predictor(Pc, Wn, pk, Wc, dU, Uxm, Uxp, Uym, Uyp, Uzm, Uzp, hcm2);
       double q[NF];
       if (wid == TY) {
         pred_state<NV>(P, Uyp, dU, q);
@@ -696,6 +705,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     }
     bc = bn;
   }
+  if (owner) cfl_rate(k1 + 1 + NG - 2);                  // the last cell written (plane k1-1)
 
   if (bad) atomicOr(s.status, 1);
   block_rate_max(rate_max, s.rate_bits);
