@@ -271,6 +271,152 @@ __device__ __forceinline__ void riemann_fs(const Phys& P, const double* L, const
 }
 
 // ------------------------------------------------------------------------------------------------
+// Batched forms: N independent instances advanced stage by stage, so that the instruction stream handed
+// to ptxas already interleaves the dependent chains (1/x and sqrt seeds + corrections, S*, fluxes).  ncu
+// showed ptxas emitting the sequential calls as sequential chains (every DFMA waiting its full latency).
+// ------------------------------------------------------------------------------------------------
+template <int N>
+__device__ __forceinline__ void rcp3_n(const double* x, double* y) {
+  double s[N], e[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(s[k]) : "d"(x[k]));
+#pragma unroll
+  for (int k = 0; k < N; ++k) e[k] = fma(-x[k], s[k], 1.0);
+#pragma unroll
+  for (int k = 0; k < N; ++k) e[k] = fma(e[k], e[k], e[k]);
+#pragma unroll
+  for (int k = 0; k < N; ++k) y[k] = fma(s[k], e[k], s[k]);
+}
+
+template <int N>
+__device__ __forceinline__ void sqrt3_n(const double* x, double* y) {
+  double s[N], t[N], e[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(s[k]) : "d"(x[k]));
+#pragma unroll
+  for (int k = 0; k < N; ++k) t[k] = x[k] * s[k];
+#pragma unroll
+  for (int k = 0; k < N; ++k) e[k] = fma(-t[k], s[k], 1.0);
+#pragma unroll
+  for (int k = 0; k < N; ++k) s[k] = fma(0.375, e[k], 0.5);
+#pragma unroll
+  for (int k = 0; k < N; ++k) e[k] = s[k] * e[k];
+#pragma unroll
+  for (int k = 0; k < N; ++k) y[k] = fma(t[k], e[k], t[k]);
+}
+
+// N predicted face states at once (same arithmetic as pred_state)
+template <int NV, int N>
+__device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q) {
+  double r[N], m1[N], m2[N], m3[N], E[N], mm[N], ir[N], e[N], x[N], c[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    r[k] = Uf[k][0] + dU[0];
+    m1[k] = Uf[k][1] + dU[1];
+    m2[k] = Uf[k][2] + dU[2];
+    m3[k] = Uf[k][3] + dU[3];
+    E[k] = Uf[k][4] + dU[4];
+  }
+  rcp3_n<N>(r, ir);
+#pragma unroll
+  for (int k = 0; k < N; ++k) mm[k] = m1[k] * m1[k];
+#pragma unroll
+  for (int k = 0; k < N; ++k) mm[k] = fma(m2[k], m2[k], mm[k]);
+#pragma unroll
+  for (int k = 0; k < N; ++k) mm[k] = fma(m3[k], m3[k], mm[k]);
+#pragma unroll
+  for (int k = 0; k < N; ++k) e[k] = fma(-0.5 * ir[k], mm[k], E[k]);
+#pragma unroll
+  for (int k = 0; k < N; ++k) x[k] = (P.gamma * P.gm1) * ir[k] * e[k];
+  sqrt3_n<N>(x, c);
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    q[k][0] = r[k];
+    q[k][1] = m1[k] * ir[k];
+    q[k][2] = m2[k] * ir[k];
+    q[k][3] = m3[k] * ir[k];
+    q[k][4] = P.gm1 * e[k];
+    q[k][5] = E[k];
+    q[k][6] = c[k];
+#pragma unroll
+    for (int s = 5; s < NV; ++s) q[k][2 + s] = (Uf[k][s] + dU[s]) * ir[k];
+  }
+}
+
+// N HLLC fluxes at once; instance k is the face normal to direction dir[k] (same arithmetic as riemann_fs)
+template <int NV, int N>
+__device__ __forceinline__ void hllc_n(const int (&dir)[N], const double* const* L, const double* const* R, double* const* F) {
+  constexpr int NF = NV + 2;
+  double uL[N], uR[N], SL[N], SR[N], dL[N], dR[N], mL[N], mR[N], num[N], den[N], Ss[N], w[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    uL[k] = L[k][1 + dir[k]];
+    uR[k] = R[k][1 + dir[k]];
+    SL[k] = fmin(uL[k] - L[k][6], uR[k] - R[k][6]);
+    SR[k] = fmax(uL[k] + L[k][6], uR[k] + R[k][6]);
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    dL[k] = SL[k] - uL[k];
+    dR[k] = SR[k] - uR[k];
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    mL[k] = L[k][0] * dL[k];
+    mR[k] = R[k][0] * dR[k];
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    den[k] = mL[k] - mR[k];
+    num[k] = fma(-uR[k], mR[k], fma(uL[k], mL[k], R[k][4] - L[k][4]));
+  }
+  rcp3_n<N>(den, w);
+#pragma unroll
+  for (int k = 0; k < N; ++k) Ss[k] = num[k] * w[k];
+  double qk[N][NF], SK[N], mK[N], dK[N], SKe[N], x[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    const bool left = (SL[k] >= 0.0) || (Ss[k] >= 0.0);
+    const bool upwind = (SL[k] >= 0.0) || (!left && SR[k] <= 0.0);   // pure F_L or F_R
+#pragma unroll
+    for (int v = 0; v < NF; ++v) qk[k][v] = left ? L[k][v] : R[k][v];
+    SK[k] = left ? SL[k] : SR[k];
+    mK[k] = left ? mL[k] : mR[k];
+    dK[k] = left ? dL[k] : dR[k];
+    SKe[k] = upwind ? 0.0 : SK[k];
+    x[k] = SK[k] - Ss[k];
+  }
+  rcp3_n<N>(x, w);
+  double fac[N], fr[N], F0[N], t1[N], t2[N], t3[N], Es[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    fac[k] = mK[k] * w[k];                               // rho*_K
+    fr[k] = qk[k][0] * qk[k][1 + dir[k]];                 // mass flux of side K
+    t3[k] = qk[k][4] * w[k];
+    t2[k] = dK[k] * w[k];
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    F0[k] = fma(SKe[k], fac[k] - qk[k][0], fr[k]);
+    t1[k] = fma(fac[k], Ss[k], -fr[k]);
+    t3[k] = fma(fac[k], Ss[k], t3[k]);
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    const double uK = qk[k][1 + dir[k]], pK = qk[k][4], EK = qk[k][5];
+    Es[k] = fma(t2[k], EK, (Ss[k] - uK) * t3[k]);         // E*_K
+    F[k][0] = F0[k];
+    F[k][1] = F0[k] * qk[k][1];
+    F[k][2] = F0[k] * qk[k][2];
+    F[k][3] = F0[k] * qk[k][3];
+    F[k][1 + dir[k]] = fma(SKe[k], t1[k], fma(fr[k], uK, pK));   // normal: F_K + S_K (rho* S* - rho_K u_K)
+    F[k][4] = fma(SKe[k], Es[k] - EK, (EK + pK) * uK);
+#pragma unroll
+    for (int s = 5; s < NV; ++s) F[k][s] = F0[k] * qk[k][2 + s];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // The kernel.  Thread roles (warp-uniform except in the last warp):
 //   warps 0..TY-1  owners of row ey = warp, cell ex = lane
 //   warp  TY       bottom ring row  ey = -1   -> provides the predicted y+ state of its cells
@@ -531,46 +677,89 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   };
 
   int bc = 1;                 // buffer of plane p
+  constexpr bool HLLC_STATIC = (RS == HX_RIEMANN_HLLC);
   for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
     const int pk = p + NG;
     const int bn = (bc == 2) ? 0 : bc + 1;
-    const bool do_xy = (p >= k0) && (p < k1);
     double* Pc = planes + bc * PSTR;
     double* Pn = planes + bn * PSTR;
     mbar_wait(&mbar[bn], (phase >> bn) & 1u);            // plane p+1 has arrived (issued a whole iteration ago)
     phase ^= (1u << bn);
 
+    // Edge iterations (p = k0-1 and p = k1) run the same code on valid but unused data; only the global
+    // store and the CFL rate are predicated, so the iteration is three straight-line blocks.
     double Wn[NV], Wc[NV], dU[NV], hcm2;
-    double Uxm[NV], Uxp[NV], Uym[NV], Uyp[NV], Uzm[NV], Uzp[NV];
+    double Uf[6][NV];          // conserved face states: 0 x-, 1 x+, 2 y-, 3 y+, 4 z-, 5 z+
     if (owner) {
-      // ======== owners: ONE straight-line block up to the first barrier, so that the slope arithmetic, the six
-      // independent predicted states, the z Riemann problem, the finish of cell p-1 and the deferred CFL rate of
-      // cell p-2 can be interleaved by the scheduler ======================================================
+      // ======== block 1: slopes, half-step increment, the six predicted states in two interleaved
+      // batches, the deferred CFL rate of cell p-2 =============================================================
       cfl_rate(pk - 2);
       convert(Pn, cidx, Wn, true);                       // [A] cons -> prim of the own cell of plane p+1, in place
-      predictor(Pc, Wn, pk, Wc, dU, Uxm, Uxp, Uym, Uyp, Uzm, Uzp, hcm2);
-      double qxm[NF], qym[NF];
+      predictor(Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2);
+      double qxm[NF], qym[NF], qzm[NF], zpn[NF];
       {
-        double q[NF];
-        pred_state<NV>(P, Uxp, dU, q);
+        double qa[NF], qb[NF];
+        const double* const ua[3] = {Uf[1], Uf[3], Uf[4]};
+        double* const qo[3] = {qa, qb, qzm};
+        pred_states<NV, 3>(P, ua, dU, qo);
 #pragma unroll
-        for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
-        pred_state<NV>(P, Uyp, dU, q);
+        for (int v = 0; v < NF; ++v) {
+          X[v * XSTR + xs_own] = qa[v];
+          Y[v * YSTR + ys_own] = qb[v];
+        }
+      }
+      {
+        const double* const ub[3] = {Uf[0], Uf[2], Uf[5]};
+        double* const qo[3] = {qxm, qym, zpn};
+        pred_states<NV, 3>(P, ub, dU, qo);
+      }
+      double Un[NV];           // U^n of cell p
+      {
+        const double rho = Wc[0];
+        Un[0] = rho;
+        Un[1] = rho * Wc[1];
+        Un[2] = rho * Wc[2];
+        Un[3] = rho * Wc[3];
+        Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), Wc[4] * P.igm1);
 #pragma unroll
-        for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
+        for (int v = 5; v < NV; ++v) Un[v] = rho * Wc[v];
       }
-      pred_state<NV>(P, Uxm, dU, qxm);
-      pred_state<NV>(P, Uym, dU, qym);
-      // ---- [C] z direction: face p-1/2, finish cell p-1, start cell p (edge iterations compute on valid
-      // but unused data; only the store and the rate are predicated) ------------------------------------
-      double Fz[NV];
-      {
-        double fzm[NF];
-        pred_state<NV>(P, Uzm, dU, fzm);
-        riemann_fs<NV, RS, 2>(P, zp, fzm, Fz);
+      asm volatile("bar.sync 0;" ::: "memory");          // (1) "+" states visible; all reads of plane p done
+      if (threadIdx.x == 0 && p + 3 <= k1 + 1) {         // plane p+3 takes the buffer of plane p
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(&mbar[bc], (uint32_t)SM::plane_bytes);
+        tma_load_plane(&tmap, Pc, &mbar[bc], xs, ys, p + 3 + NG);
       }
-      pred_state<NV>(P, Uzp, dU, zp);
+      // ======== block 2: the three Riemann problems on the lower faces of this cell (x and y fluxes go back into
+      // the slots), finish cell p-1 with the z flux, start cell p =============================================
+      double Fx[NV], Fy[NV], Fz[NV];
       {
+        double qlx[NF], qly[NF];
+#pragma unroll
+        for (int v = 0; v < NF; ++v) {
+          qlx[v] = X[v * XSTR + xs_nbr];
+          qly[v] = Y[v * YSTR + ys_nbr];
+        }
+        if (HLLC_STATIC) {
+          const int dirs[3] = {0, 1, 2};
+          const double* const Ls[3] = {qlx, qly, zp};
+          const double* const Rs[3] = {qxm, qym, qzm};
+          double* const Fs[3] = {Fx, Fy, Fz};
+          hllc_n<NV, 3>(dirs, Ls, Rs, Fs);
+        } else {
+          riemann_fs<NV, RS, 0>(P, qlx, qxm, Fx);
+          riemann_fs<NV, RS, 1>(P, qly, qym, Fy);
+          riemann_fs<NV, RS, 2>(P, zp, qzm, Fz);
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          X[v * XSTR + xs_nbr] = Fx[v];
+          Y[v * YSTR + ys_nbr] = Fy[v];
+        }
+      }
+#pragma unroll
+      for (int v = 0; v < NF; ++v) zp[v] = zpn[v];
+      {   // the flux through the upper z face of cell p-1 is Fz: write the cell once
         const double k2p = 2.0 * (UNI ? a.uhc[2] : c2p * __ldg(T.cf[2][1][2] + pk - 1));
         double Unew[NV];
 #pragma unroll
@@ -600,83 +789,47 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
         for (int v = 0; v < 5; ++v) Ul[v] = Unew[v];
       }
-      {   // U^n of cell p + the lower z face
-        const double rho = Wc[0];
-        const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
-        double Un[NV];
-        Un[0] = rho;
-        Un[1] = mcx;
-        Un[2] = mcy;
-        Un[3] = mcz;
-        Un[4] = fma(0.5, fma(mcz, Wc[3], fma(mcy, Wc[2], mcx * Wc[1])), Wc[4] * P.igm1);
-#pragma unroll
-        for (int v = 5; v < NV; ++v) Un[v] = rho * Wc[v];
+      {   // cell p: U^n + the three lower faces
         const double k2m = 2.0 * hcm2;
 #pragma unroll
-        for (int v = 0; v < NV; ++v) Up[v] = fma(k2m, Fz[v], Un[v]);
+        for (int v = 0; v < NV; ++v) {
+          double u = fma(k2m, Fz[v], Un[v]);
+          u = fma((SPH && (v == 2 || v == 3)) ? kxm : k0m, Fx[v], u);
+          Up[v] = fma((SPH && v == 3) ? kym : k1m, Fy[v], u);
+        }
         if (SPH) {
-          Up[1] = fma(hgr, Fz[3], Up[1]);
+          Up[1] = fma(hgr, Fz[3] + Fy[2], Up[1]);
           Up[2] = fma(hcgt, Fz[3], Up[2]);
         }
         if (GRAV != GRAV_OFF) {
-          Un0 = rho;
-          Unm[0] = mcx;
-          Unm[1] = mcy;
-          Unm[2] = mcz;
+          Un0 = Un[0];
+          Unm[0] = Un[1];
+          Unm[1] = Un[2];
+          Unm[2] = Un[3];
         }
-      }
-      asm volatile("bar.sync 0;" ::: "memory");          // (1) "+" states visible; all reads of plane p done
-      if (threadIdx.x == 0 && p + 3 <= k1 + 1) {         // plane p+3 takes the buffer of plane p
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_expect_tx(&mbar[bc], (uint32_t)SM::plane_bytes);
-        tma_load_plane(&tmap, Pc, &mbar[bc], xs, ys, p + 3 + NG);
-      }
-      // ---- [E] x and y faces on the lower side of this cell: Riemann flux once, back into the slot -----
-      if (do_xy) {
-        double qlx[NF], qly[NF], Fx[NV], Fy[NV];
-#pragma unroll
-        for (int v = 0; v < NF; ++v) {
-          qlx[v] = X[v * XSTR + xs_nbr];
-          qly[v] = Y[v * YSTR + ys_nbr];
-        }
-        riemann_fs<NV, RS, 0>(P, qlx, qxm, Fx);
-        riemann_fs<NV, RS, 1>(P, qly, qym, Fy);
-#pragma unroll
-        for (int v = 0; v < NV; ++v) {
-          X[v * XSTR + xs_nbr] = Fx[v];
-          Y[v * YSTR + ys_nbr] = Fy[v];
-        }
-#pragma unroll
-        for (int v = 0; v < NV; ++v) {
-          Up[v] = fma((SPH && (v == 2 || v == 3)) ? kxm : k0m, Fx[v], Up[v]);
-          Up[v] = fma((SPH && v == 3) ? kym : k1m, Fy[v], Up[v]);
-        }
-        if (SPH) Up[1] = fma(hgr, Fy[2], Up[1]);
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (2) fluxes visible
-      // ---- [F] fluxes through the upper x and y faces come back in the own slots -----------------------
-      if (do_xy) {
+      // ======== block 3: fluxes through the upper x and y faces come back in the own slots ================
 #pragma unroll
-        for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? kxp : k0p), X[v * XSTR + xs_own], Up[v]);
-        if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
+      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? kxp : k0p), X[v * XSTR + xs_own], Up[v]);
+      if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? kyp : k1p), Y[v * YSTR + ys_own], Up[v]);
-      }
+      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? kyp : k1p), Y[v * YSTR + ys_own], Up[v]);
     } else {
       // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
       convert_plane(Pn, Wn);
-      predictor(Pc, Wn, pk, Wc, dU, Uxm, Uxp, Uym, Uyp, Uzm, Uzp, hcm2);
+      predictor(Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2);
       double q[NF];
       if (wid == TY) {
-        pred_state<NV>(P, Uyp, dU, q);
+        pred_state<NV>(P, Uf[3], dU, q);
 #pragma unroll
         for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
       } else if (wid == TY + 1) {
-        pred_state<NV>(P, Uym, dU, q);
+        pred_state<NV>(P, Uf[2], dU, q);
       } else {
         double Us[NV];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) Us[v] = (ex < 0) ? Uxp[v] : Uxm[v];
+        for (int v = 0; v < NV; ++v) Us[v] = (ex < 0) ? Uf[1][v] : Uf[0][v];
         pred_state<NV>(P, Us, dU, q);
         if (wr_px) {
 #pragma unroll
@@ -684,22 +837,20 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         }
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (1)
-      if (do_xy) {
-        if (wid == TY + 1) {
-          double ql[NF], F[NV];
+      if (wid == TY + 1) {
+        double ql[NF], F[NV];
 #pragma unroll
-          for (int v = 0; v < NF; ++v) ql[v] = Y[v * YSTR + ys_nbr];
-          riemann_fs<NV, RS, 1>(P, ql, q, F);
+        for (int v = 0; v < NF; ++v) ql[v] = Y[v * YSTR + ys_nbr];
+        riemann_fs<NV, RS, 1>(P, ql, q, F);
 #pragma unroll
-          for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
-        } else if (do_rx) {
-          double ql[NF], F[NV];
+        for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
+      } else if (do_rx) {
+        double ql[NF], F[NV];
 #pragma unroll
-          for (int v = 0; v < NF; ++v) ql[v] = X[v * XSTR + xs_nbr];
-          riemann_fs<NV, RS, 0>(P, ql, q, F);
+        for (int v = 0; v < NF; ++v) ql[v] = X[v * XSTR + xs_nbr];
+        riemann_fs<NV, RS, 0>(P, ql, q, F);
 #pragma unroll
-          for (int v = 0; v < NV; ++v) X[v * XSTR + xs_nbr] = F[v];
-        }
+        for (int v = 0; v < NV; ++v) X[v * XSTR + xs_nbr] = F[v];
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (2)
     }
