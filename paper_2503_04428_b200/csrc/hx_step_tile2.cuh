@@ -86,17 +86,22 @@ __device__ __forceinline__ double sqrt3(double x) {   // x > 0
 }
 
 __device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
+// plain compare-select minimum / maximum (no NaN quieting: inputs are finite wherever the result is used)
+__device__ __forceinline__ double dmin(double a, double b) { return (a < b) ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return (a > b) ? a : b; }
+// true when a and b have opposite sign bits
+__device__ __forceinline__ bool opp_sign(double a, double b) { return ((hi32(a) ^ hi32(b)) & 0x80000000) != 0; }
 
 // limiter on one-sided differences a (backward), b (forward); all are homogeneous of degree 1
 template <int LIM>
 __device__ __forceinline__ double lim_core(int lim_rt, double a, double b) {
   if (LIM == HX_LIM_MINMOD) {
-    const bool opp = (hi32(a) ^ hi32(b)) < 0;
+    const bool opp = opp_sign(a, b);
     const double r = (fabs(a) < fabs(b)) ? a : b;
     return opp ? 0.0 : r;
   }
   if (LIM == HX_LIM_MC) {
-    const bool opp = (hi32(a) ^ hi32(b)) < 0;
+    const bool opp = opp_sign(a, b);
     const double c = 0.5 * (a + b);
     const double m = (fabs(a) < fabs(b)) ? a : b;
     const double m2 = m + m;
@@ -219,8 +224,8 @@ template <int NV, int RS, int DIR>
 __device__ __forceinline__ void riemann_fs(const Phys& P, const double* L, const double* R, double* F) {
   constexpr int NF = NV + 2;
   const double uL = L[1 + DIR], uR = R[1 + DIR];
-  const double SL = fmin(uL - L[6], uR - R[6]);
-  const double SR = fmax(uL + L[6], uR + R[6]);
+  const double SL = dmin(uL - L[6], uR - R[6]);
+  const double SR = dmax(uL + L[6], uR + R[6]);
   const bool hllc = (RS == HX_RIEMANN_HLLC) || (RS < 0 && P.riemann == HX_RIEMANN_HLLC);
   if (hllc) {
     const double dL = SL - uL, dR = SR - uR;
@@ -352,8 +357,8 @@ __device__ __forceinline__ void hllc_n(const int (&dir)[N], const double* const*
   for (int k = 0; k < N; ++k) {
     uL[k] = L[k][1 + dir[k]];
     uR[k] = R[k][1 + dir[k]];
-    SL[k] = fmin(uL[k] - L[k][6], uR[k] - R[k][6]);
-    SR[k] = fmax(uL[k] + L[k][6], uR[k] + R[k][6]);
+    SL[k] = dmin(uL[k] - L[k][6], uR[k] - R[k][6]);
+    SR[k] = dmax(uL[k] + L[k][6], uR[k] + R[k][6]);
   }
 #pragma unroll
   for (int k = 0; k < N; ++k) {
@@ -606,7 +611,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     const double il2 = UNI ? a.uil[2] : il2xy * __ldg(T.lf[2][2] + pkc);
     const double rate = fma(fma(fabs(Ul[1]), ir, cs), il0, fma(fma(fabs(Ul[2]), ir, cs), il1, fma(fabs(Ul[3]), ir, cs) * il2));
     const bool fine = (Ul[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL));
-    rate_max = (st_l && fine) ? fmax(rate_max, rate) : rate_max;
+    rate_max = (st_l && fine && rate > rate_max) ? rate : rate_max;
     bad = bad || (st_l && !fine);
   };
 
