@@ -25,6 +25,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "hx_common.cuh"
 
 namespace hx {
@@ -35,7 +37,19 @@ constexpr int PX = TX + 4;    // staged plane row: tile + 2 ghost cells on each 
 #ifndef HX_T2_TY
 #define HX_T2_TY 8
 #endif
-constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows + 3 ring warps = 11 warps: two owner warps per scheduler, ring warps spread over three
+constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows (two warpgroups) + 4 ring warps (one warpgroup): two owner warps and one ring warp per scheduler
+
+// Register budgets after setmaxnreg.  The pool is what the CTA was given at launch, (TY+4) warps x 32 x REGS_LAUNCH
+// (not the whole 64 K file): the owners' increase must fit into what the ring warpgroup releases, or
+// setmaxnreg.inc waits forever.
+#ifndef HX_T2_REGS_RING
+#define HX_T2_REGS_RING 96
+#endif
+constexpr int REGS_RING = HX_T2_REGS_RING;
+constexpr int REGS_LAUNCH = (65536 / ((TY_DEFAULT + 4) * 32)) / 8 * 8;
+constexpr int REGS_OWNER_RAW = (REGS_LAUNCH * (TY_DEFAULT + 4) - REGS_RING * 4) / TY_DEFAULT / 8 * 8;
+constexpr int REGS_OWNER = REGS_OWNER_RAW > 232 ? 232 : REGS_OWNER_RAW;
+static_assert(REGS_OWNER * TY_DEFAULT + REGS_RING * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
 
 enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2 };   // GRAV_Z: acceleration along direction 2 only
 
@@ -426,12 +440,16 @@ __device__ __forceinline__ void hllc_n(const int (&dir)[N], const double* const*
 //   warps 0..TY-1  owners of row ey = warp, cell ex = lane
 //   warp  TY       bottom ring row  ey = -1   -> provides the predicted y+ state of its cells
 //   warp  TY+1     top ring row     ey = TY   -> solves the y face below it
-//   warp  TY+2     lanes 0..15 left ring column ex = -1 (x+ state), lanes 16..31 right ring column ex = TX (x face)
+//   warp  TY+2     left ring column  ex = -1  (lanes 0..TY-1)  -> provides the predicted x+ state
+//   warp  TY+3     right ring column ex = TX  (lanes 0..TY-1)  -> solves the x face on its left
+// The owner warps and the ring warps form separate warpgroups and rebalance the register file with
+// setmaxnreg: the ring path needs far fewer registers than it is given at launch, and ptxas interleaves the
+// independent fp64 chains of the owner path only when it has ~200 registers (at 168 it emits them serially).
 // ------------------------------------------------------------------------------------------------
 template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int TY>
-__global__ void __launch_bounds__((TY + 3) * 32, 1)
+__global__ void __launch_bounds__((TY + 4) * 32, 1)
 step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Args a) {
-  static_assert(TY >= 1 && TY <= 16, "the side-ring warp holds two columns of at most 16 cells");
+  static_assert(TY % 4 == 0 && TY >= 4 && TY <= 32, "owner warps must fill whole warpgroups (setmaxnreg)");
   static_assert(!(UNI && SPH), "UNI is for Cartesian grids");
   using SM = Smem<NV, TY>;
   constexpr int NF = SM::NF, FSTR = SM::FSTR, XSTR = SM::XSTR, YSTR = SM::YSTR, XP = SM::XP;
@@ -465,14 +483,12 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     xoff = PX;
     coff = (lane == 0) ? -1 : (lane == 31 ? 1 : 0);
   } else {
-    const int l = lane & 15;
-    ex = (lane >> 4) ? TX : -1;
-    ey = min(l, TY - 1);
-    act = l < TY;
-    xoff = (lane >> 4) ? 1 : -1;
+    const bool right = wid == TY + 3;
+    ex = right ? TX : -1;
+    ey = min(lane, TY - 1);
+    act = lane < TY;
+    xoff = right ? 1 : -1;
   }
-  const bool wr_px = (owner || (wid == TY + 2 && ex < 0)) && act;      // writes its predicted x+ state
-  const bool do_rx = (owner || (wid == TY + 2 && ex >= TX)) && act;    // solves the x face on its lower side
 
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
   const int k0 = blockIdx.z * a.zc, k1 = min(L.n[2], k0 + a.zc);
@@ -681,8 +697,10 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     }
   };
 
-  int bc = 1;                 // buffer of plane p
   constexpr bool HLLC_STATIC = (RS == HX_RIEMANN_HLLC);
+  auto march = [&](auto own_tag) {
+  constexpr bool OWN = decltype(own_tag)::value;
+  int bc = 1;                 // buffer of plane p
   for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
     const int pk = p + NG;
     const int bn = (bc == 2) ? 0 : bc + 1;
@@ -695,7 +713,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // store and the CFL rate are predicated, so the iteration is three straight-line blocks.
     double Wn[NV], Wc[NV], dU[NV], hcm2;
     double Uf[6][NV];          // conserved face states: 0 x-, 1 x+, 2 y-, 3 y+, 4 z-, 5 z+
-    if (owner) {
+    if constexpr (OWN) {
       // ======== block 1: slopes, half-step increment, the six predicted states in two interleaved
       // batches, the deferred CFL rate of cell p-2 =============================================================
       cfl_rate(pk - 2);
@@ -831,15 +849,14 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
       } else if (wid == TY + 1) {
         pred_state<NV>(P, Uf[2], dU, q);
-      } else {
-        double Us[NV];
-#pragma unroll
-        for (int v = 0; v < NV; ++v) Us[v] = (ex < 0) ? Uf[1][v] : Uf[0][v];
-        pred_state<NV>(P, Us, dU, q);
-        if (wr_px) {
+      } else if (wid == TY + 2) {
+        pred_state<NV>(P, Uf[1], dU, q);
+        if (act) {
 #pragma unroll
           for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
         }
+      } else {
+        pred_state<NV>(P, Uf[0], dU, q);
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (1)
       if (wid == TY + 1) {
@@ -849,7 +866,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         riemann_fs<NV, RS, 1>(P, ql, q, F);
 #pragma unroll
         for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
-      } else if (do_rx) {
+      } else if (wid == TY + 3 && act) {
         double ql[NF], F[NV];
 #pragma unroll
         for (int v = 0; v < NF; ++v) ql[v] = X[v * XSTR + xs_nbr];
@@ -861,7 +878,15 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     }
     bc = bn;
   }
-  if (owner) cfl_rate(k1 + 1 + NG - 2);                  // the last cell written (plane k1-1)
+  };
+  if (owner) {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_OWNER));
+    march(std::true_type{});
+    cfl_rate(k1 + 1 + NG - 2);                           // the last cell written (plane k1-1)
+  } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_RING));
+    march(std::false_type{});
+  }
 
   if (bad) atomicOr(s.status, 1);
   block_rate_max(rate_max, s.rate_bits);

@@ -30,7 +30,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t s
     attr_set = true;
   }
   plan.name = UNI ? "tile2_uni" : "tile2";
-  kern<<<plan.grid, (TY + 3) * 32, Smem<NV, TY>::total, st>>>(plan.tmap[cur], a);
+  kern<<<plan.grid, (TY + 4) * 32, Smem<NV, TY>::total, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();
 }
 
