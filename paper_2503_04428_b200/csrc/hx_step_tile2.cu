@@ -38,11 +38,28 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], 
   Plan* p = new Plan();
   constexpr int TY = t2::TY_DEFAULT;
   const int ntx = (L.n[0] + t2::TX - 1) / t2::TX, nty = (L.n[1] + TY - 1) / TY;
-  // z chunks: about 8 CTAs per SM over the whole grid so that the tail of the last wave stays small, chunks of at
-  // least 32 planes (each chunk re-reads 4 planes and recomputes 2 predictor planes)
-  int nzc = 1;
+  // z chunks: every chunk re-reads 4 planes and recomputes 2 predictor planes (+ a prologue), and with one CTA per
+  // SM the grid runs in waves of `sms` CTAs of equal length: pick the chunk count that maximises
+  // (useful planes / planes marched) x (waves / whole waves).
+  int sms = 148;
+  {
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess && prop.multiProcessorCount > 0)
+      sms = prop.multiProcessorCount;
+  }
   const long long cols = (long long)ntx * nty;
-  while (cols * nzc < 148LL * 8 && L.n[2] / (nzc + 1) >= 32) ++nzc;
+  int nzc = 1;
+  double best = -1.0;
+  for (int c = 1; c <= (L.n[2] + 15) / 16; ++c) {
+    const int zc = (L.n[2] + c - 1) / c, chunks = (L.n[2] + zc - 1) / zc;
+    const double waves = (double)(cols * chunks) / sms;
+    const double eff = (double)L.n[2] / ((double)chunks * (zc + 3)) * waves / (double)(long long)(waves + 0.999999);
+    if (eff > best + 1e-9) {
+      best = eff;
+      nzc = chunks;
+    }
+  }
   p->zc = (L.n[2] + nzc - 1) / nzc;
   nzc = (L.n[2] + p->zc - 1) / p->zc;
   p->grid = dim3((unsigned)ntx, (unsigned)nty, (unsigned)nzc);

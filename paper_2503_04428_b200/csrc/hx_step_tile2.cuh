@@ -42,14 +42,20 @@ constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows (two warpgroups) + 4 ring
 // Register budgets after setmaxnreg.  The pool is what the CTA was given at launch, (TY+4) warps x 32 x REGS_LAUNCH
 // (not the whole 64 K file): the owners' increase must fit into what the ring warpgroup releases, or
 // setmaxnreg.inc waits forever.
-#ifndef HX_T2_REGS_RING
-#define HX_T2_REGS_RING 96
+// Measured (A/B on B200): ring 96..120 is equal for the Cartesian builds; the spherical ring path (nine fields,
+// geometric sources) spills below ~136 and then holds the owners up at the barriers (5.0 -> 6.6 Gcell/s).
+#ifdef HX_T2_REGS_RING
+constexpr int ring_regs(bool) { return HX_T2_REGS_RING; }
+#else
+constexpr int ring_regs(bool sph) { return sph ? 136 : 120; }
 #endif
-constexpr int REGS_RING = HX_T2_REGS_RING;
 constexpr int REGS_LAUNCH = (65536 / ((TY_DEFAULT + 4) * 32)) / 8 * 8;
-constexpr int REGS_OWNER_RAW = (REGS_LAUNCH * (TY_DEFAULT + 4) - REGS_RING * 4) / TY_DEFAULT / 8 * 8;
-constexpr int REGS_OWNER = REGS_OWNER_RAW > 232 ? 232 : REGS_OWNER_RAW;
-static_assert(REGS_OWNER * TY_DEFAULT + REGS_RING * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+constexpr int owner_regs(bool sph) {
+  const int raw = (REGS_LAUNCH * (TY_DEFAULT + 4) - ring_regs(sph) * 4) / TY_DEFAULT / 8 * 8;
+  return raw > 232 ? 232 : raw;
+}
+static_assert(owner_regs(true) * TY_DEFAULT + ring_regs(true) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(false) * TY_DEFAULT + ring_regs(false) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
 
 enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2 };   // GRAV_Z: acceleration along direction 2 only
 
@@ -125,11 +131,12 @@ __device__ __forceinline__ double lim_core(int lim_rt, double a, double b) {
   return limited_slope(LIM < 0 ? lim_rt : LIM, a, b);
 }
 
-// hw * lim(dm * idx_lo, dp * idx_hi)  (Eq. 17 with R5); fl = hw*idx_lo, fh = hw*idx_hi
+// hw * lim(dm * idx_lo, dp * idx_hi)  (Eq. 17 with R5); fl = hw*idx_lo, fh = hw*idx_hi.  On uniform grids
+// (fl == fh) the common factor is left to the caller, who folds it into the face-state FMA.
 template <int LIM, bool UNI>
 __device__ __forceinline__ double lim_pre(int lim_rt, double dm, double dp, double fl, double fh) {
   if (LIM == HX_LIM_NONE) return 0.0;
-  if (UNI) return fl * lim_core<LIM>(lim_rt, dm, dp);
+  if (UNI) return lim_core<LIM>(lim_rt, dm, dp);
   return lim_core<LIM>(lim_rt, dm * fl, dp * fh);
 }
 
@@ -181,14 +188,14 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
   for (int s = 5; s < NV; ++s) W[s] = U[s] * ir;
 }
 
-// One face of the cell along DIR: face primitives Wc + sgn t (Eq. 17), their conserved form Uf, and the
+// One face of the cell along DIR: face primitives Wc + sc t (Eq. 17; sc = -+1, or -+hw*idx on uniform grids), their conserved form Uf, and the
 // analytic flux of that state accumulated into the half-step increment dU with the signed, (dt/2)-scaled
 // area/volume coefficient `coef` (Eq. 18: + for the lower face, - for the upper face).
-template <int NV, int DIR, bool PLUS>
-__device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double coef, double* Uf, double* dU) {
+template <int NV, int DIR>
+__device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double sc, double coef, double* Uf, double* dU) {
   double Wf[NV];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) Wf[v] = PLUS ? (Wc[v] + t[v]) : (Wc[v] - t[v]);
+  for (int v = 0; v < NV; ++v) Wf[v] = fma(sc, t[v], Wc[v]);
   const double r = Wf[0];
   Uf[0] = r;
   Uf[1] = r * Wf[1];
@@ -656,23 +663,23 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
     }
-    face_cons_flux<NV, 0, false>(P, Wc, t, hcm0, Uxm, dU);
-    face_cons_flux<NV, 0, true>(P, Wc, t, -hcp0, Uxp, dU);
+    face_cons_flux<NV, 0>(P, Wc, t, UNI ? -flx : -1.0, hcm0, Uxm, dU);
+    face_cons_flux<NV, 0>(P, Wc, t, UNI ? flx : 1.0, -hcp0, Uxp, dU);
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
     }
-    face_cons_flux<NV, 1, false>(P, Wc, t, hcm1, Uym, dU);
-    face_cons_flux<NV, 1, true>(P, Wc, t, -hcp1, Uyp, dU);
+    face_cons_flux<NV, 1>(P, Wc, t, UNI ? -fly : -1.0, hcm1, Uym, dU);
+    face_cons_flux<NV, 1>(P, Wc, t, UNI ? fly : 1.0, -hcp1, Uyp, dU);
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const double dp = Wn[v] - Wc[v];
       t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
       dzm[v] = dp;
     }
-    face_cons_flux<NV, 2, false>(P, Wc, t, hcm2, Uzm, dU);
-    face_cons_flux<NV, 2, true>(P, Wc, t, -hcp2, Uzp, dU);
+    face_cons_flux<NV, 2>(P, Wc, t, UNI ? -flz : -1.0, hcm2, Uzm, dU);
+    face_cons_flux<NV, 2>(P, Wc, t, UNI ? flz : 1.0, -hcp2, Uzp, dU);
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
@@ -880,11 +887,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   }
   };
   if (owner) {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_OWNER));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(owner_regs(SPH)));
     march(std::true_type{});
     cfl_rate(k1 + 1 + NG - 2);                           // the last cell written (plane k1-1)
   } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_RING));
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ring_regs(SPH)));
     march(std::false_type{});
   }
 
