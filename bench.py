@@ -213,7 +213,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     sim = hx.Hydro(spec, stream=stream)
     if args.kernel != "auto":
-        sim.set_option(hx.OPT_KERNEL, {"generic": hx.KERNEL_GENERIC, "tiled_v1": hx.KERNEL_TILED, "tile2": hx.KERNEL_TILE2}[args.kernel])
+        sim.set_option(hx.OPT_KERNEL, {"generic": hx.KERNEL_GENERIC, "tile2": hx.KERNEL_TILED}[args.kernel])
     W = np.ascontiguousarray(W)
     sim.set_state(W, hx.PRIMITIVE)
     U0 = sim.get_state()                      # conserved initial state (host) for the e2e leg
@@ -319,7 +319,7 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled_v1", "tile2"], help="step kernel (A/B runs)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tile2"], help="step kernel (A/B runs)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of CPU oracle timing")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

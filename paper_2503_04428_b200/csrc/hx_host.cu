@@ -16,12 +16,6 @@ cudaError_t launch_unpack(const Layout& L, const Phys& P, const double* U, doubl
 cudaError_t launch_rate(const Layout& L, const Tables& T, const Phys& P, const double* U, unsigned long long* rate_bits, int* status,
                         cudaStream_t s);
 cudaError_t launch_step_generic(const StepArgs& a, cudaStream_t s);
-struct TiledPlan;
-int tiled_supported(const Layout& L, const Phys& P);
-cudaError_t tiled_plan_create(const Layout& L, const Phys& P, double* const U[2], TiledPlan** out);
-void tiled_plan_destroy(TiledPlan* p);
-cudaError_t launch_step_tiled(TiledPlan* plan, const StepArgs& a, int cur, cudaStream_t s);
-const char* tiled_kernel_name(const TiledPlan* p);
 namespace t2 { struct Plan; }
 int tile2_supported(const Layout& L, const Phys& P);
 cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, t2::Plan** out);
@@ -51,8 +45,6 @@ struct hx_handle {
   cudaStream_t stream = nullptr;
   bool rate_valid = false;
   int kernel_opt = HX_KERNEL_AUTO;
-  TiledPlan* plan = nullptr;
-  bool plan_tried = false;
   t2::Plan* plan2 = nullptr;
   bool plan2_tried = false;
   bool uniform = false;       // Cartesian grid whose per-axis tables are bitwise constant
@@ -373,7 +365,6 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
 
 int hx_destroy(hx_handle* h) {
   if (!h) return HX_OK;
-  if (h->plan) tiled_plan_destroy(h->plan);
   if (h->plan2) tile2_plan_destroy(h->plan2);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
@@ -395,9 +386,8 @@ int hx_set_stream(hx_handle* h, void* cuda_stream) {
 int hx_set_option(hx_handle* h, int option, int value) {
   if (!h) return HX_ERR_INVALID_ARG;
   if (option == HX_OPT_KERNEL) {
-    if (value < HX_KERNEL_AUTO || value > HX_KERNEL_TILE2) return fail(h, HX_ERR_INVALID_ARG, "unknown kernel selection");
-    if (value == HX_KERNEL_TILED && !tiled_supported(h->L, h->P)) return fail(h, HX_ERR_UNSUPPORTED, "the tiled kernel does not cover this configuration");
-    if (value == HX_KERNEL_TILE2 && !tile2_supported(h->L, h->P)) return fail(h, HX_ERR_UNSUPPORTED, "the tile2 kernel does not cover this configuration");
+    if (value < HX_KERNEL_AUTO || value > HX_KERNEL_TILED) return fail(h, HX_ERR_INVALID_ARG, "unknown kernel selection");
+    if (value == HX_KERNEL_TILED && !tile2_supported(h->L, h->P)) return fail(h, HX_ERR_UNSUPPORTED, "the tiled kernel does not cover this configuration");
     h->kernel_opt = value;
     return HX_OK;
   }
@@ -509,9 +499,9 @@ int hx_step(hx_handle* h, double dt) {
   e = cudaMemsetAsync(&h->d_scal->rate_bits, 0, sizeof(unsigned long long), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: memset");
   StepArgs a = make_args(h, dt);
-  bool use_tiled = false, use_tile2 = false;
+  bool use_tile2 = false;
   const int ko = h->kernel_opt;
-  if ((ko == HX_KERNEL_AUTO || ko == HX_KERNEL_TILE2) && tile2_supported(L, h->P)) {
+  if ((ko == HX_KERNEL_AUTO || ko == HX_KERNEL_TILED) && tile2_supported(L, h->P)) {
     if (!h->plan2 && !h->plan2_tried) {
       h->plan2_tried = true;
       const int grav_z = h->cfg.gravity == HX_GRAV_UNIFORM && h->cfg.g[0] == 0.0 && h->cfg.g[1] == 0.0;
@@ -523,26 +513,12 @@ int hx_step(hx_handle* h, double dt) {
     }
     use_tile2 = h->plan2 != nullptr;
     if (!use_tile2) return fail(h, HX_ERR_CUDA, "tile2 kernel unavailable");
-  } else if (ko == HX_KERNEL_TILED && tiled_supported(L, h->P)) {
-    if (!h->plan && !h->plan_tried) {
-      h->plan_tried = true;
-      e = tiled_plan_create(L, h->P, h->d_U, &h->plan);
-      if (e != cudaSuccess) {
-        h->plan = nullptr;
-        return cuda_fail(h, e, "hx_step: tiled plan");
-      }
-    }
-    use_tiled = h->plan != nullptr;
-    if (!use_tiled) return fail(h, HX_ERR_CUDA, "tiled kernel unavailable");
   }
   const bool timed = h->timing && !h->ev_pending;
   if (timed) cudaEventRecord(h->ev0, h->stream);
   if (use_tile2) {
     e = launch_step_tile2(h->plan2, a, h->cur, h->stream);
     h->last_kernel = tile2_kernel_name(h->plan2);
-  } else if (use_tiled) {
-    e = launch_step_tiled(h->plan, a, h->cur, h->stream);
-    h->last_kernel = tiled_kernel_name(h->plan);
   } else {
     e = launch_step_generic(a, h->stream);
     h->last_kernel = "generic";

@@ -49,10 +49,15 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], 
       sms = prop.multiProcessorCount;
   }
   const long long cols = (long long)ntx * nty;
-  int nzc = 1;
+  // the chunk's z tables live in shared memory next to the plane ring and the exchange buffers (227 KB per CTA)
+  const size_t plane = ((size_t)L.nvar * (TY + 4) * t2::PX * 8 + 127) / 128 * 128;
+  const size_t fixed = 3 * plane + (size_t)(L.nvar + 2) * (TY * (t2::TX + 2) + (TY + 1) * t2::TX) * 8 + 192;
+  const size_t budget = 227 * 1024 - 1024;   // static shared memory of the block reduction + reserve
+  int nzc = (L.n[2] + 15) / 16;
   double best = -1.0;
   for (int c = 1; c <= (L.n[2] + 15) / 16; ++c) {
     const int zc = (L.n[2] + c - 1) / c, chunks = (L.n[2] + zc - 1) / zc;
+    if (fixed + 6 * (size_t)(zc + 6) * 8 > budget) continue;
     const double waves = (double)(cols * chunks) / sms;
     const double eff = (double)L.n[2] / ((double)chunks * (zc + 3)) * waves / (double)(long long)(waves + 0.999999);
     if (eff > best + 1e-9) {

@@ -81,7 +81,8 @@ struct Smem {
   static constexpr int YSTR = (TY + 1) * TX;                   // y-exchange: slots ey = -1 .. TY-1
   static constexpr size_t x_bytes = (size_t)NF * XSTR * sizeof(double);
   static constexpr size_t y_bytes = (size_t)NF * YSTR * sizeof(double);
-  static constexpr size_t total = NPL * plane_stride + x_bytes + y_bytes + 64 + 128;
+  static constexpr size_t fixed = NPL * plane_stride + x_bytes + y_bytes + 64 + 128;
+  static constexpr size_t total(int zc) { return fixed + 6 * (size_t)(zc + 6) * sizeof(double); }   // + z tables of one chunk
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -467,6 +468,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   double* X = (double*)(base + SM::NPL * SM::plane_stride);
   double* Y = X + NF * XSTR;
   uint64_t* mbar = (uint64_t*)(Y + NF * YSTR);
+  double* zt = (double*)(mbar + 8);   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
 
   const StepArgs& s = a.s;
   const Layout& L = s.L;
@@ -562,6 +564,18 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     mbar_init(&mbar[2], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // padded z indices touched by this chunk: k0-3+NG (deferred CFL rate of the first iteration, unused) .. k1+1+NG
+  const int zb = max(k0 - 3 + NG, 0), zlen = a.zc + 6;
+  for (int q = threadIdx.x; q < zlen; q += blockDim.x) {
+    const int pz = min(zb + q, L.np[2] - 1);
+    zt[q] = T.hw[2][pz];
+    zt[zlen + q] = T.idx[2][pz];
+    zt[2 * zlen + q] = T.cf[2][0][2][pz];
+    zt[3 * zlen + q] = T.cf[2][1][2][pz];
+    zt[4 * zlen + q] = T.grav[2][pz];
+    zt[5 * zlen + q] = T.lf[2][2][pz];
+  }
+  auto ZT = [&](int k, int pz) { return zt[k * zlen + (pz - zb)]; };
   __syncthreads();
   if (threadIdx.x == 0) {
 #pragma unroll
@@ -631,7 +645,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     const double ir = rcp3(Ul[0]);
     const double e = fma(-0.5 * ir, mm, Ul[4]);
     const double cs = sqrt3((P.gamma * P.gm1) * ir * e);
-    const double il2 = UNI ? a.uil[2] : il2xy * __ldg(T.lf[2][2] + pkc);
+    const double il2 = UNI ? a.uil[2] : il2xy * ZT(5, max(pkc, zb));
     const double rate = fma(fma(fabs(Ul[1]), ir, cs), il0, fma(fma(fabs(Ul[2]), ir, cs), il1, fma(fabs(Ul[3]), ir, cs) * il2));
     const bool fine = (Ul[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL));
     rate_max = (st_l && fine && rate > rate_max) ? rate : rate_max;
@@ -646,11 +660,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       flz = fhz = a.uf[2];
       hcm2 = hcp2 = a.uhc[2];
     } else {
-      const double hwz = __ldg(T.hw[2] + pk);
-      flz = hwz * __ldg(T.idx[2] + pk);
-      fhz = hwz * __ldg(T.idx[2] + pk + 1);
-      hcm2 = c2m * __ldg(T.cf[2][0][2] + pk);
-      hcp2 = c2p * __ldg(T.cf[2][1][2] + pk);
+      const double hwz = ZT(0, pk);
+      flz = hwz * ZT(1, pk);
+      fhz = hwz * ZT(1, pk + 1);
+      hcm2 = c2m * ZT(2, pk);
+      hcp2 = c2p * ZT(3, pk);
     }
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
@@ -694,7 +708,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       dU[4] = fma(mcx, hgx, fma(mcy, hgy, dU[4]));
     }
     if (GRAV != GRAV_OFF) {
-      const double hgz = hdt * __ldg(T.grav[2] + pk);
+      const double hgz = hdt * ZT(4, pk);
       dU[3] = fma(rho, hgz, dU[3]);
       dU[4] = fma(mcz, hgz, dU[4]);
     }
@@ -790,7 +804,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
       for (int v = 0; v < NF; ++v) zp[v] = zpn[v];
       {   // the flux through the upper z face of cell p-1 is Fz: write the cell once
-        const double k2p = 2.0 * (UNI ? a.uhc[2] : c2p * __ldg(T.cf[2][1][2] + pk - 1));
+        const double k2p = 2.0 * (UNI ? a.uhc[2] : c2p * ZT(3, pk - 1));
         double Unew[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) Unew[v] = fma(-k2p, Fz[v], Up[v]);
@@ -799,7 +813,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Unew[2] = fma(hcgt, Fz[3], Unew[2]);
         }
         if (GRAV != GRAV_OFF) {   // time-centred (R13)
-          const double hgzp = hdt * __ldg(T.grav[2] + pk - 1);
+          const double hgzp = hdt * ZT(4, pk - 1);
           const double rs = Un0 + Unew[0];
           if (GRAV == GRAV_ANY) {
             const double m1 = fma(rs, hgx, Unew[1]), m2 = fma(rs, hgy, Unew[2]);

@@ -23,14 +23,15 @@ template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI>
 static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   constexpr int TY = TY_DEFAULT;
   auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Smem<NV, TY>::total);
+  const size_t smem = Smem<NV, TY>::total(plan.zc);
+  static size_t attr_set = 0;
+  if (attr_set < smem) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    attr_set = smem;
   }
   plan.name = UNI ? "tile2_uni" : "tile2";
-  kern<<<plan.grid, (TY + 4) * 32, Smem<NV, TY>::total, st>>>(plan.tmap[cur], a);
+  kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();
 }
 

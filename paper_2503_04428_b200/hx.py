@@ -23,7 +23,7 @@ SPACING_UNIFORM, SPACING_LOG, SPACING_CUSTOM = 0, 1, 2
 HOST, DEVICE = 0, 1
 CONSERVED, PRIMITIVE = 0, 1
 OPT_KERNEL, OPT_TIMING = 0, 1
-KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_TILE2 = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 EXPORTS = ["hx_create", "hx_destroy", "hx_set_stream", "hx_set_option", "hx_set_state", "hx_get_state",
            "hx_compute_dt", "hx_step", "hx_nvar", "hx_launch_count", "hx_kernel_time", "hx_step_kernel_name", "hx_last_error",

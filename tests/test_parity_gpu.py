@@ -16,7 +16,6 @@ pytestmark = pytest.mark.gpu
 TOL_STEP = 1e-12
 TOL_L1 = 1e-9
 KERNELS = ["generic", "auto"]
-KERNELS_3D = KERNELS + ["tiled_v1"]     # the first tiled design stays selectable for A/B runs
 
 
 @pytest.fixture(scope="module")
@@ -32,8 +31,6 @@ def make_pair(hx, ox, spec, W, kernel="auto"):
     g = hx.Hydro(spec)
     if kernel == "generic":
         g.set_option(hx.OPT_KERNEL, hx.KERNEL_GENERIC)
-    elif kernel == "tiled_v1" and spec["ndim"] == 3:
-        g.set_option(hx.OPT_KERNEL, hx.KERNEL_TILED)
     g.set_state(np.ascontiguousarray(W), hx.PRIMITIVE)
     o = ox.Oracle(spec)
     o.set_state(W, ox.PRIMITIVE)
@@ -62,7 +59,7 @@ REDUCED = {
 }
 
 
-@pytest.mark.parametrize("kernel", KERNELS_3D)
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("name", list(REDUCED))
 def test_one_step_parity(hx, oxlib, name, kernel):
     ox = oxlib
@@ -81,7 +78,7 @@ def test_one_step_parity(hx, oxlib, name, kernel):
     assert abs(dt_g2 - dt_o2) <= 1e-12 * dt_o2
 
 
-@pytest.mark.parametrize("kernel", KERNELS_3D)
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("name", list(REDUCED))
 def test_hundred_step_parity(hx, oxlib, name, kernel):
     ox = oxlib
