@@ -63,7 +63,7 @@ struct Args {
   StepArgs s;
   int zc;            // planes per z chunk
   // UNI instantiations only (bitwise-uniform Cartesian tables): constants of the three axes
-  double uf[3];      // hw * idx   (slope pre-scale, = 1/2 up to rounding)
+  double uf[3];      // hw * idx   (slope pre-scale, = 1/2 up to rounding), times the limiter's lim_scale (1/2 for MC)
   double uhc[3];     // (dt/2) / delta_d
   double uil[3];     // 1 / delta_d  (CFL inverse lengths)
 };
@@ -106,6 +106,10 @@ __device__ __forceinline__ double sqrt3(double x) {   // x > 0
   return fma(t, q, t);
 }
 
+// scale the caller applies to what lim_core returns
+template <int LIM>
+__device__ __forceinline__ constexpr double lim_scale() { return LIM == HX_LIM_MC ? 0.5 : 1.0; }
+
 __device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
 // plain compare-select minimum / maximum (no NaN quieting: inputs are finite wherever the result is used)
 __device__ __forceinline__ double dmin(double a, double b) { return (a < b) ? a : b; }
@@ -121,12 +125,12 @@ __device__ __forceinline__ double lim_core(int lim_rt, double a, double b) {
     const double r = (fabs(a) < fabs(b)) ? a : b;
     return opp ? 0.0 : r;
   }
-  if (LIM == HX_LIM_MC) {
+  if (LIM == HX_LIM_MC) {   // returns TWICE the limited value (the caller's face scale carries the 1/2): saves a multiply
     const bool opp = opp_sign(a, b);
-    const double c = 0.5 * (a + b);
+    const double sum = a + b;
     const double m = (fabs(a) < fabs(b)) ? a : b;
-    const double m2 = m + m;
-    const double r = (fabs(m2) < fabs(c)) ? m2 : c;
+    const double m4 = 4.0 * m;
+    const double r = (fabs(m4) < fabs(sum)) ? m4 : sum;   // 2 min(2|a|, 2|b|, |a+b|/2) with the common sign
     return opp ? 0.0 : r;
   }
   return limited_slope(LIM < 0 ? lim_rt : LIM, a, b);
@@ -677,23 +681,23 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
     }
-    face_cons_flux<NV, 0>(P, Wc, t, UNI ? -flx : -1.0, hcm0, Uxm, dU);
-    face_cons_flux<NV, 0>(P, Wc, t, UNI ? flx : 1.0, -hcp0, Uxp, dU);
+    face_cons_flux<NV, 0>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU);
+    face_cons_flux<NV, 0>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU);
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
     }
-    face_cons_flux<NV, 1>(P, Wc, t, UNI ? -fly : -1.0, hcm1, Uym, dU);
-    face_cons_flux<NV, 1>(P, Wc, t, UNI ? fly : 1.0, -hcp1, Uyp, dU);
+    face_cons_flux<NV, 1>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU);
+    face_cons_flux<NV, 1>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU);
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       const double dp = Wn[v] - Wc[v];
       t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
       dzm[v] = dp;
     }
-    face_cons_flux<NV, 2>(P, Wc, t, UNI ? -flz : -1.0, hcm2, Uzm, dU);
-    face_cons_flux<NV, 2>(P, Wc, t, UNI ? flz : 1.0, -hcp2, Uzp, dU);
+    face_cons_flux<NV, 2>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU);
+    face_cons_flux<NV, 2>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU);
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
