@@ -197,7 +197,8 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
 // analytic flux of that state accumulated into the half-step increment dU with the signed, (dt/2)-scaled
 // area/volume coefficient `coef` (Eq. 18: + for the lower face, - for the upper face).
 template <int NV, int DIR>
-__device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double sc, double coef, double* Uf, double* dU) {
+__device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double sc, double coef, double* Uf, double* dU,
+                                               double* unc_out = nullptr) {
   double Wf[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) Wf[v] = fma(sc, t[v], Wc[v]);
@@ -209,6 +210,7 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
   const double ke2 = fma(Uf[3], Wf[3], fma(Uf[2], Wf[2], Uf[1] * Wf[1]));
   Uf[4] = fma(0.5, ke2, Wf[4] * P.igm1);
   const double unc = Wf[1 + DIR] * coef;
+  if (unc_out) *unc_out = unc;   // signed (dt/2) dS/dV u_n of this face: what a passive scalar's flux rides on
   dU[0] = fma(r, unc, dU[0]);
   dU[1] = fma(Uf[1], unc, dU[1]);
   dU[2] = fma(Uf[2], unc, dU[2]);
@@ -338,7 +340,7 @@ __device__ __forceinline__ void sqrt3_n(const double* x, double* y) {
 
 // N predicted face states at once (same arithmetic as pred_state)
 template <int NV, int N>
-__device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q) {
+__device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q, double* const* ir_out = nullptr) {
   double r[N], m1[N], m2[N], m3[N], E[N], mm[N], ir[N], e[N], x[N], c[N];
 #pragma unroll
   for (int k = 0; k < N; ++k) {
@@ -369,6 +371,7 @@ __device__ __forceinline__ void pred_states(const Phys& P, const double* const* 
     q[k][4] = P.gm1 * e[k];
     q[k][5] = E[k];
     q[k][6] = c[k];
+    if (ir_out) *ir_out[k] = ir[k];
 #pragma unroll
     for (int s = 5; s < NV; ++s) q[k][2 + s] = (Uf[k][s] + dU[s]) * ir[k];
   }
@@ -657,8 +660,12 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   };
 
   // [B] O2-O4 for the cell of plane p: limited slopes, face states, half-step increment dU (Eq. 17-18, unsplit)
-  auto predictor = [&](const double* Pc, const double* Wn, int pk, double* Wc, double* dU, double* Uxm, double* Uxp, double* Uym,
-                       double* Uyp, double* Uzm, double* Uzp, double& hcm2) {
+  // nvp_tag: how many leading fields it handles (all of them for the ring warps; the five hydro fields for the
+  // owners, whose passive scalars follow one at a time to keep the register peak down); unc6: per-face signed
+  // (dt/2) dS/dV u_n for that scalar pass.
+  auto predictor = [&](auto nvp_tag, const double* Pc, const double* Wn, int pk, double* Wc, double* dU, double* Uxm, double* Uxp,
+                       double* Uym, double* Uyp, double* Uzm, double* Uzp, double& hcm2, double* unc6) {
+    constexpr int NVP = decltype(nvp_tag)::value;
     double flz, fhz, hcp2;   // per-plane z geometry (uniform addresses)
     if (UNI) {
       flz = fhz = a.uf[2];
@@ -671,33 +678,33 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       hcp2 = c2p * ZT(3, pk);
     }
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NVP; ++v) {
       Wc[v] = Pc[v * FSTR + cidx];
       dU[v] = 0.0;
     }
-    double t[NV];
+    double t[NVP];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
     }
-    face_cons_flux<NV, 0>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU);
-    face_cons_flux<NV, 0>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU);
+    face_cons_flux<NVP, 0>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU, unc6 ? unc6 + 0 : nullptr);
+    face_cons_flux<NVP, 0>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU, unc6 ? unc6 + 1 : nullptr);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
     }
-    face_cons_flux<NV, 1>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU);
-    face_cons_flux<NV, 1>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU);
+    face_cons_flux<NVP, 1>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU, unc6 ? unc6 + 2 : nullptr);
+    face_cons_flux<NVP, 1>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU, unc6 ? unc6 + 3 : nullptr);
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NVP; ++v) {
       const double dp = Wn[v] - Wc[v];
       t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
       dzm[v] = dp;
     }
-    face_cons_flux<NV, 2>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU);
-    face_cons_flux<NV, 2>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU);
+    face_cons_flux<NVP, 2>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, unc6 ? unc6 + 4 : nullptr);
+    face_cons_flux<NVP, 2>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, unc6 ? unc6 + 5 : nullptr);
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
@@ -718,7 +725,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     }
     if (lim_none) {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) dU[v] = 0.0;
+      for (int v = 0; v < NVP; ++v) dU[v] = 0.0;
     }
   };
 
@@ -743,15 +750,17 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       // batches, the deferred CFL rate of cell p-2 =============================================================
       cfl_rate(pk - 2);
       convert(Pn, cidx, Wn, true);                       // [A] cons -> prim of the own cell of plane p+1, in place
-      predictor(Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2);
+      double unc[6], ir6[6];   // per face: signed (dt/2) dS/dV u_n of the face state, 1/rho of the predicted state
+      predictor(std::integral_constant<int, 5>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, unc);
       double qxm[NF], qym[NF], qzm[NF], zpn[NF];
       {
         double qa[NF], qb[NF];
         const double* const ua[3] = {Uf[1], Uf[3], Uf[4]};
         double* const qo[3] = {qa, qb, qzm};
-        pred_states<NV, 3>(P, ua, dU, qo);
+        double* const io[3] = {&ir6[1], &ir6[3], &ir6[4]};
+        pred_states<5, 3>(P, ua, dU, qo, io);
 #pragma unroll
-        for (int v = 0; v < NF; ++v) {
+        for (int v = 0; v < 7; ++v) {
           X[v * XSTR + xs_own] = qa[v];
           Y[v * YSTR + ys_own] = qb[v];
         }
@@ -759,7 +768,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       {
         const double* const ub[3] = {Uf[0], Uf[2], Uf[5]};
         double* const qo[3] = {qxm, qym, zpn};
-        pred_states<NV, 3>(P, ub, dU, qo);
+        double* const io[3] = {&ir6[0], &ir6[2], &ir6[5]};
+        pred_states<5, 3>(P, ub, dU, qo, io);
       }
       double Un[NV];           // U^n of cell p
       {
@@ -769,8 +779,48 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         Un[2] = rho * Wc[2];
         Un[3] = rho * Wc[3];
         Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), Wc[4] * P.igm1);
+      }
+      if constexpr (NV > 5) {
+        // Passive scalars one at a time (R7: mass fractions are reconstructed, rho f is advanced): limited slopes,
+        // the six face values, the scalar's own half-step increment from the face mass fluxes kept in `unc`, and
+        // the predicted mass fraction on every face.  Same arithmetic as the all-fields predictor of the ring path.
+        double flz, fhz;
+        if (UNI) {
+          flz = fhz = a.uf[2];
+        } else {
+          const double hwz = ZT(0, pk);
+          flz = hwz * ZT(1, pk);
+          fhz = hwz * ZT(1, pk + 1);
+        }
+        const double scx = UNI ? flx : lim_scale<LIM>(), scy = UNI ? fly : lim_scale<LIM>(), scz = UNI ? flz : lim_scale<LIM>();
 #pragma unroll
-        for (int v = 5; v < NV; ++v) Un[v] = rho * Wc[v];
+        for (int sv = 5; sv < NV; ++sv) {
+          const double* Ps = Pc + sv * FSTR + cidx;
+          const double fc = Ps[0];
+          const double tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, flx, fhx);
+          const double ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, fly, fhy);
+          const double dp = Pn[sv * FSTR + cidx] - fc;
+          const double tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
+          dzm[sv] = dp;
+          double rf[6];
+          rf[0] = Uf[0][0] * fma(-scx, tx, fc);
+          rf[1] = Uf[1][0] * fma(scx, tx, fc);
+          rf[2] = Uf[2][0] * fma(-scy, ty, fc);
+          rf[3] = Uf[3][0] * fma(scy, ty, fc);
+          rf[4] = Uf[4][0] * fma(-scz, tz, fc);
+          rf[5] = Uf[5][0] * fma(scz, tz, fc);
+          double dUs = 0.0;
+#pragma unroll
+          for (int k = 0; k < 6; ++k) dUs = fma(rf[k], unc[k], dUs);
+          if (lim_none) dUs = 0.0;
+          X[(2 + sv) * XSTR + xs_own] = (rf[1] + dUs) * ir6[1];
+          Y[(2 + sv) * YSTR + ys_own] = (rf[3] + dUs) * ir6[3];
+          qxm[2 + sv] = (rf[0] + dUs) * ir6[0];
+          qym[2 + sv] = (rf[2] + dUs) * ir6[2];
+          qzm[2 + sv] = (rf[4] + dUs) * ir6[4];
+          zpn[2 + sv] = (rf[5] + dUs) * ir6[5];
+          Un[sv] = Wc[0] * fc;
+        }
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (1) "+" states visible; all reads of plane p done
       if (threadIdx.x == 0 && p + 3 <= k1 + 1) {         // plane p+3 takes the buffer of plane p
@@ -866,7 +916,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     } else {
       // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
       convert_plane(Pn, Wn);
-      predictor(Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2);
+      predictor(std::integral_constant<int, NV>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, nullptr);
       double q[NF];
       if (wid == TY) {
         pred_state<NV>(P, Uf[3], dU, q);
