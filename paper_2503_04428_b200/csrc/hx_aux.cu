@@ -5,54 +5,92 @@
 
 namespace hx {
 
-// One direction of the ordered ghost fill.  Work item = (field, transverse cell, side, layer).
-// Transverse extent: full padded range for directions already filled (e < d), interior range
-// for directions still to come (e > d) -- identical result to sweeping the full padded extent
-// because later passes overwrite those cells anyway.
-__global__ void ghost_fill_kernel(Layout L, double* __restrict__ U, int d, int bc_lo, int bc_hi) {
-  int ext[3], base[3];
-  for (int e = 0; e < 3; ++e) {
-    if (e < d) { ext[e] = L.np[e]; base[e] = 0; }
-    else { ext[e] = L.n[e]; base[e] = L.ng[e]; }
+// Ghost fill (A0), all directions in ONE launch.  The ordered fill "direction 0, then 1, then 2, each pass
+// spanning the ghosts of the earlier ones" gives every ghost cell the value of the interior
+// cell found by mapping each out-of-range index back into the interior with that direction's boundary
+// condition (periodic: wrap; null gradient: clamp; reflective: mirror and flip the normal momentum) -- the maps
+// of different directions commute, so the composition is evaluated directly: one read, one write per ghost cell.
+struct GhostBC {
+  int lo[3], hi[3];
+};
+
+__device__ __forceinline__ int ghost_src(int i, int n, int bc_lo, int bc_hi, bool& flip) {
+  if (i < 0) {
+    const int g = -i;
+    if (bc_lo == HX_BC_PERIODIC) return n - g;
+    if (bc_lo == HX_BC_TRANSMISSIVE) return 0;
+    flip = !flip;
+    return g - 1;
   }
-  ext[d] = 2 * NG;   // side * NG + layer
-  const long long per_field = (long long)ext[0] * ext[1] * ext[2];
-  const long long total = per_field * L.nvar;
-  const int n = L.n[d];
+  if (i >= n) {
+    const int g = i - n + 1;
+    if (bc_hi == HX_BC_PERIODIC) return g - 1;
+    if (bc_hi == HX_BC_TRANSMISSIVE) return n - 1;
+    flip = !flip;
+    return n - g;
+  }
+  return i;
+}
+
+// Work items: three disjoint slab groups that cover the ghost shell --
+//   A: ghost in direction 0, any padded (q1, q2);  B: interior in 0, ghost in 1, any padded q2;  C: interior in 0 and 1, ghost in 2.
+__global__ void ghost_fill_kernel(Layout L, double* __restrict__ U, GhostBC bc) {
+  const int G0 = 2 * L.ng[0], G1 = 2 * L.ng[1], G2 = 2 * L.ng[2];
+  const long long nA = (long long)G0 * L.np[1] * L.np[2];
+  const long long nB = (long long)L.n[0] * G1 * L.np[2];
+  const long long nC = (long long)L.n[0] * L.n[1] * G2;
+  const long long per_field = nA + nB + nC, total = per_field * L.nvar;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
     const int v = (int)(t / per_field);
     long long r = t % per_field;
-    int c[3];
-    c[0] = (int)(r % ext[0]); r /= ext[0];
-    c[1] = (int)(r % ext[1]); r /= ext[1];
-    c[2] = (int)r;
-    const int side = c[d] / NG, g = c[d] % NG + 1;   // g = 1, 2: distance from the boundary face
-    const int bc = side ? bc_hi : bc_lo;
-    int src, dst;
-    if (side == 0) {
-      dst = -g;
-      src = (bc == HX_BC_PERIODIC) ? n - g : (bc == HX_BC_TRANSMISSIVE ? 0 : g - 1);
+    int q[3];   // padded indices of the ghost cell
+    if (r < nA) {
+      const int c = (int)(r % G0);
+      r /= G0;
+      q[0] = c < L.ng[0] ? c : L.n[0] + c;            // ghosts below: 0..ng-1, above: n+ng..n+2ng-1
+      q[1] = (int)(r % L.np[1]);
+      q[2] = (int)(r / L.np[1]);
+    } else if (r < nA + nB) {
+      r -= nA;
+      q[0] = (int)(r % L.n[0]) + L.ng[0];
+      r /= L.n[0];
+      const int c = (int)(r % G1);
+      q[1] = c < L.ng[1] ? c : L.n[1] + c;
+      q[2] = (int)(r / G1);
     } else {
-      dst = n - 1 + g;
-      src = (bc == HX_BC_PERIODIC) ? g - 1 : (bc == HX_BC_TRANSMISSIVE ? n - 1 : n - g);
+      r -= nA + nB;
+      q[0] = (int)(r % L.n[0]) + L.ng[0];
+      r /= L.n[0];
+      q[1] = (int)(r % L.n[1]) + L.ng[1];
+      const int c = (int)(r / L.n[1]);
+      q[2] = c < L.ng[2] ? c : L.n[2] + c;
     }
-    int p[3] = {c[0] + base[0], c[1] + base[1], c[2] + base[2]};
-    p[d] = src + NG;
-    double val = U[v * L.sv + L.off(p[0], p[1], p[2])];
-    if ((bc == HX_BC_REFLECTING || bc == HX_BC_WEDGE) && v == 1 + d) val = -val;
-    p[d] = dst + NG;
-    U[v * L.sv + L.off(p[0], p[1], p[2])] = val;
+    int src[3];
+    bool neg = false;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      bool flip = false;
+      src[d] = ghost_src(q[d] - L.ng[d], L.n[d], bc.lo[d], bc.hi[d], flip) + L.ng[d];
+      if (flip && v == 1 + d && d < L.ndim) neg = !neg;
+    }
+    const double val = U[v * L.sv + L.off(src[0], src[1], src[2])];
+    U[v * L.sv + L.off(q[0], q[1], q[2])] = neg ? -val : val;
   }
 }
 
-cudaError_t launch_ghost_fill(const Layout& L, double* U, int d, int bc_lo, int bc_hi, cudaStream_t s) {
-  long long total = (long long)L.nvar * 2 * NG;
-  for (int e = 0; e < 3; ++e)
-    if (e != d) total *= (e < d) ? L.np[e] : L.n[e];
+cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, const int* bc_hi, cudaStream_t s) {
+  GhostBC bc;
+  for (int d = 0; d < 3; ++d) {
+    bc.lo[d] = bc_lo[d];
+    bc.hi[d] = bc_hi[d];
+  }
+  const long long per_field = 2LL * L.ng[0] * L.np[1] * L.np[2] + 2LL * L.n[0] * L.ng[1] * L.np[2] + 2LL * L.n[0] * L.n[1] * L.ng[2];
+  const long long total = per_field * L.nvar;
+  if (total == 0) return cudaSuccess;
   const int block = 256;
   long long grid = (total + block - 1) / block;
-  if (grid > 148LL * 16) grid = 148LL * 16;
-  ghost_fill_kernel<<<(unsigned)grid, block, 0, s>>>(L, U, d, bc_lo, bc_hi);
+  if (grid > 148LL * 32) grid = 148LL * 32;
+  ghost_fill_kernel<<<(unsigned)grid, block, 0, s>>>(L, U, bc);
   return cudaGetLastError();
 }
 

@@ -10,7 +10,7 @@
 #include "hx_common.cuh"
 
 namespace hx {
-cudaError_t launch_ghost_fill(const Layout& L, double* U, int d, int bc_lo, int bc_hi, cudaStream_t s);
+cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, const int* bc_hi, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const Phys& P, const double* src, double* U, int to_cons, cudaStream_t s);
 cudaError_t launch_unpack(const Layout& L, const Phys& P, const double* U, double* dst, int to_prim, cudaStream_t s);
 cudaError_t launch_rate(const Layout& L, const Tables& T, const Phys& P, const double* U, unsigned long long* rate_bits, int* status,
@@ -491,11 +491,9 @@ int hx_step(hx_handle* h, double dt) {
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, HX_ERR_INVALID_ARG, "dt must be positive and finite");
   const Layout& L = h->L;
   cudaError_t e;
-  for (int d = 0; d < L.ndim; ++d) {   // A0, ordered 0 -> 1 -> 2
-    e = launch_ghost_fill(L, h->d_U[h->cur], d, h->cfg.bc_lo[d], h->cfg.bc_hi[d], h->stream);
-    if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: ghost fill");
-    h->launches++;
-  }
+  e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);   // A0: all directions, one launch
+  if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: ghost fill");
+  h->launches++;
   e = cudaMemsetAsync(&h->d_scal->rate_bits, 0, sizeof(unsigned long long), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: memset");
   StepArgs a = make_args(h, dt);
