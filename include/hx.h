@@ -83,10 +83,11 @@ int hx_set_state(hx_handle* h, const double* data, int mem_space, int form);
 int hx_get_state(hx_handle* h, double* data, int mem_space, int form);
 /* A7: dt = cfl / max over interior cells of sum_d (|u_d|+c_s)/l_d (R2).  Uses the rate
  * the last hx_step folded into its update when available, else runs the reduction kernel.
- * Synchronises the stream (one 16-byte device-to-host copy). */
+ * One 16-byte device-to-host copy; waits for the last step kernel (not for the ghost fill hx_step queues behind it)
+ * or, right after hx_set_state, for the reduction kernel. */
 int hx_compute_dt(hx_handle* h, double cfl, double* dt_out);
-/* A0-A6 (+A7 fused): ghost fill, then one unsplit MUSCL-Hancock / Godunov update of every interior
- * cell by dt (Eq. 17-19, sources Eq. 13-16, gravity Eq. 2-3).  Asynchronous on the stream; device
+/* A0-A6 (+A7 fused): ghost fill (done eagerly at the end of the previous hx_step when there was one), then one
+ * unsplit MUSCL-Hancock / Godunov update of every interior cell by dt (Eq. 17-19, sources Eq. 13-16, gravity Eq. 2-3).  Asynchronous on the stream; device
  * side errors surface at the next hx_compute_dt / hx_get_state. */
 int hx_step(hx_handle* h, double dt);
 /* Number of stored fields, 2 + ndim + n_scalars. */

@@ -43,6 +43,9 @@ struct hx_handle {
   DevScalars* d_scal = nullptr;
   DevScalars* h_scal = nullptr;   // pinned
   cudaStream_t stream = nullptr;
+  cudaStream_t side = nullptr;    // reads the CFL rate back while the next ghost fill already runs on `stream`
+  cudaEvent_t ev_step = nullptr;  // recorded right after the step kernel
+  bool ghosts_valid = false;      // ghost layers of d_U[cur] are filled (hx_step fills them eagerly for the next step)
   bool rate_valid = false;
   int kernel_opt = HX_KERNEL_AUTO;
   t2::Plan* plan2 = nullptr;
@@ -356,6 +359,8 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
   if (e == cudaSuccess) e = cudaMemset(h->d_scal, 0, sizeof(DevScalars));
   if (e == cudaSuccess) e = cudaMallocHost(&h->h_scal, sizeof(DevScalars));
   if (e != cudaSuccess) { hx_destroy(h); return HX_ERR_ALLOC; }
+  if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&h->ev_step, cudaEventDisableTiming) != cudaSuccess) { hx_destroy(h); return HX_ERR_CUDA; }
   const int rc = build_tables(h);
   if (rc != HX_OK) { hx_destroy(h); return rc; }
   h->cfg.faces[0] = h->cfg.faces[1] = h->cfg.faces[2] = nullptr;   // caller arrays are not retained
@@ -366,6 +371,8 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
 int hx_destroy(hx_handle* h) {
   if (!h) return HX_OK;
   if (h->plan2) tile2_plan_destroy(h->plan2);
+  if (h->side) cudaStreamDestroy(h->side);
+  if (h->ev_step) cudaEventDestroy(h->ev_step);
   if (h->ev0) cudaEventDestroy(h->ev0);
   if (h->ev1) cudaEventDestroy(h->ev1);
   for (int b = 0; b < 2; ++b)
@@ -433,6 +440,7 @@ int hx_set_state(hx_handle* h, const double* data, int mem_space, int form) {
   e = cudaMemsetAsync(h->d_scal, 0, sizeof(DevScalars), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_set_state: memset");
   h->rate_valid = false;
+  h->ghosts_valid = false;
   if (mem_space == HX_HOST) {
     e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_set_state: sync");
@@ -466,7 +474,9 @@ int hx_compute_dt(hx_handle* h, double cfl, double* dt_out) {
   if (!h || !dt_out) return HX_ERR_INVALID_ARG;
   if (!(cfl > 0.0)) return fail(h, HX_ERR_INVALID_ARG, "cfl must be positive");
   cudaError_t e;
+  bool ran_rate_kernel = false;
   if (!h->rate_valid) {
+    ran_rate_kernel = true;
     e = cudaMemsetAsync(&h->d_scal->rate_bits, 0, sizeof(unsigned long long), h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_compute_dt: memset");
     e = launch_rate(h->L, h->T, h->P, h->d_U[h->cur], &h->d_scal->rate_bits, &h->d_scal->status, h->stream);
@@ -474,8 +484,16 @@ int hx_compute_dt(hx_handle* h, double cfl, double* dt_out) {
     h->launches++;
     h->rate_valid = true;
   }
-  e = cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(DevScalars), cudaMemcpyDeviceToHost, h->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (ran_rate_kernel) {
+    e = cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(DevScalars), cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  } else {
+    // the rate was folded in by the last step kernel: read it back on the side stream, which waits for that kernel
+    // only, so the ghost fill hx_step already queued for the next step keeps the GPU busy meanwhile
+    e = cudaStreamWaitEvent(h->side, h->ev_step, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(DevScalars), cudaMemcpyDeviceToHost, h->side);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->side);
+  }
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_compute_dt: sync");
   collect_timing(h);
   if (h->h_scal->status & 1) return fail(h, HX_ERR_NONPHYSICAL, "non-physical state (rho <= 0, P <= 0 or non-finite)");
@@ -491,9 +509,11 @@ int hx_step(hx_handle* h, double dt) {
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, HX_ERR_INVALID_ARG, "dt must be positive and finite");
   const Layout& L = h->L;
   cudaError_t e;
-  e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);   // A0: all directions, one launch
-  if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: ghost fill");
-  h->launches++;
+  if (!h->ghosts_valid) {   // A0: all directions, one launch (normally done eagerly at the end of the previous hx_step)
+    e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: ghost fill");
+    h->launches++;
+  }
   e = cudaMemsetAsync(&h->d_scal->rate_bits, 0, sizeof(unsigned long long), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: memset");
   StepArgs a = make_args(h, dt);
@@ -529,6 +549,13 @@ int hx_step(hx_handle* h, double dt) {
   h->launches++;
   h->cur = 1 - h->cur;
   h->rate_valid = true;
+  // The next step needs the ghost layers of the new state whatever its dt will be: fill them now, behind the event
+  // hx_compute_dt waits for, so that the host's read-back of the CFL rate overlaps this kernel.
+  e = cudaEventRecord(h->ev_step, h->stream);
+  if (e == cudaSuccess) e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: eager ghost fill");
+  h->launches++;
+  h->ghosts_valid = true;
   return HX_OK;
 }
 
