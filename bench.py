@@ -39,6 +39,7 @@ WORKLOADS = {
     "rt_3d": (lambda: wl.rt_3d(512), lambda: wl.rt_3d((96, 96, 96))),
     "sedov_3d": (lambda: wl.sedov_3d(256), lambda: wl.sedov_3d((96, 96, 96))),
     "wedge_3d": (lambda: wl.wedge_3d((1024, 256, 256)), lambda: wl.wedge_3d((192, 48, 48))),
+    "sedov_wedge_3d": (lambda: wl.sedov_wedge_3d(256), lambda: wl.sedov_wedge_3d(64)),   # PAPER.md Sect. 4.3
     "kh_2d": (lambda: wl.kh_2d(1024), lambda: wl.kh_2d(512)),
     "sod_1d": (lambda: wl.sod_1d(1000), lambda: wl.sod_1d(1000)),
     # small case for quick checks of this script
@@ -182,6 +183,20 @@ def aggregate_max_ms(local_ms, world, backend_device=None):
     return float(t.item())
 
 
+LIMITERS = {"none": wl.LIM_NONE, "minmod": wl.LIM_MINMOD, "vanleer": wl.LIM_VANLEER, "vanalbada": wl.LIM_VANALBADA, "mc": wl.LIM_MC}
+SOLVERS = {"hll": wl.RIEMANN_HLL, "hllc": wl.RIEMANN_HLLC}
+
+
+def override(problem, args):
+    spec, W = problem
+    spec = dict(spec)
+    if args.limiter:
+        spec["limiter"] = LIMITERS[args.limiter]
+    if args.riemann:
+        spec["riemann"] = SOLVERS[args.riemann]
+    return spec, W
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -203,6 +218,9 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     make_full, make_reduced = WORKLOADS[args.workload]
+    if args.limiter or args.riemann:       # measured variants of a workload: other limiter / solver
+        mf, mr = make_full, make_reduced
+        make_full, make_reduced = (lambda: override(mf(), args)), (lambda: override(mr(), args))
     spec, W = make_full()
     if world > 1:   # independent replicas: same structure, rank-specific noise
         spec, W = make_full() if rank == 0 else WORKLOADS[args.workload][0]()
@@ -290,7 +308,7 @@ def run_ours(args):
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "grid": spec["n"][:spec["ndim"]], "nvar": nvar, "cells": ncell,
-                   "scheme": "unsplit MUSCL-Hancock + HLLC, fp64", "cfl": cfl, "step_kernel": kernel_name,
+                   "scheme": "unsplit MUSCL-Hancock + %s + %s, fp64" % ({v: k for k, v in SOLVERS.items()}[spec["riemann"]], {v: k for k, v in LIMITERS.items()}[spec["limiter"]]), "cfl": cfl, "step_kernel": kernel_name,
                    "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no sharding, SURVEY 8(e))",
                    "l2": f"inputs larger than L2 (two state buffers = {state_gb:.1f} GB vs 126 MB L2)" if state_gb > 0.5
                          else "state fits in L2: HBM fraction not meaningful for this workload"},
@@ -319,6 +337,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--limiter", default=None, choices=sorted(LIMITERS), help="override the workload's slope limiter")
+    ap.add_argument("--riemann", default=None, choices=sorted(SOLVERS), help="override the workload's Riemann solver")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tile2"], help="step kernel (A/B runs)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of CPU oracle timing")
     args = ap.parse_args()

@@ -133,7 +133,17 @@ __device__ __forceinline__ double lim_core(int lim_rt, double a, double b) {
     const double r = (fabs(m4) < fabs(sum)) ? m4 : sum;   // 2 min(2|a|, 2|b|, |a+b|/2) with the common sign
     return opp ? 0.0 : r;
   }
-  return limited_slope(LIM < 0 ? lim_rt : LIM, a, b);
+  // van Leer 2ab/(a+b), van Albada ab(a+b)/(a^2+b^2) (R4), zero across extrema; the runtime-switch build (LIM < 0)
+  // dispatches here on a warp-uniform value.  Reciprocals by seed + cubic correction instead of IEEE division.
+  const int lim = LIM < 0 ? lim_rt : LIM;
+  if (lim == HX_LIM_NONE) return 0.0;
+  if (lim == HX_LIM_MINMOD) return lim_core<HX_LIM_MINMOD>(lim_rt, a, b);
+  if (lim == HX_LIM_MC) return 0.5 * lim_core<HX_LIM_MC>(lim_rt, a, b);
+  const double ab = a * b;
+  double r;
+  if (lim == HX_LIM_VANLEER) r = 2.0 * ab * rcp3(a + b);
+  else r = ab * (a + b) * rcp3(fma(a, a, b * b));
+  return (ab > 0.0) ? r : 0.0;
 }
 
 // hw * lim(dm * idx_lo, dp * idx_hi)  (Eq. 17 with R5); fl = hw*idx_lo, fh = hw*idx_hi.  On uniform grids
@@ -838,7 +848,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           qlx[v] = X[v * XSTR + xs_nbr];
           qly[v] = Y[v * YSTR + ys_nbr];
         }
-        if (HLLC_STATIC) {
+        if (HLLC_STATIC || (RS < 0 && P.riemann == HX_RIEMANN_HLLC)) {
           const int dirs[3] = {0, 1, 2};
           const double* const Ls[3] = {qlx, qly, zp};
           const double* const Rs[3] = {qxm, qym, qzm};

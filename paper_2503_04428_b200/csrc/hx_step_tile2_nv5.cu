@@ -1,4 +1,5 @@
-// NV = 5 (3-D, no passive scalar).  Fully specialised: Cartesian, no gravity, minmod + HLLC (config 3, sedov_3d).
+// NV = 5 (3-D, no passive scalar).  Fully specialised: no gravity, minmod + HLLC, Cartesian (config 3, sedov_3d) and
+// spherical (the paper's off-centre Sedov wedge, Sect. 4.3).
 #include "hx_step_tile2_launch.cuh"
 namespace hx {
 namespace t2 {
@@ -9,6 +10,8 @@ cudaError_t launch_nv<5>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
     if (plan.uni) return launch_cfg<5, false, GRAV_OFF, HX_LIM_MINMOD, HX_RIEMANN_HLLC, true>(plan, a, cur, st);
     return launch_cfg<5, false, GRAV_OFF, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);
   }
+  if (P.spherical && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
+    return launch_cfg<5, true, GRAV_OFF, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);
   return launch_generic<5>(plan, a, cur, st);
 }
 }  // namespace t2

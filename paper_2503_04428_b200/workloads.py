@@ -186,6 +186,36 @@ def wedge_3d(n=(1024, 256, 256), seed=1005):
     return spec, W
 
 
+def sedov_wedge_3d(n=256, t_end=0.08):
+    """SURVEY 8(f) rank 3, the paper's own spherical workload (Sect. 4.3): off-centre Sedov
+    blast in a spherical wedge r in [0.1, 1.3], theta and phi in [pi/4, 3pi/4], 256^3 zones, rho0 = 1, P0 = 0.01,
+    E1 = 1 at (r0, theta0, phi0) = (0.7, pi/2, pi/2), transmissive faces, gamma 5/3, run to t = 0.08.  The paper
+    does not say how E1 is deposited, nor limiter / solver / CFL: here it is thermal energy spread uniformly (per
+    volume) over the cells whose centre lies within 3.5 radial cell widths of the blast point, with minmod + HLLC
+    at CFL 0.6 like the Cartesian Sedov configuration.  No noise: the setup is deterministic."""
+    nr, nt, nph = (n, n, n) if np.isscalar(n) else n
+    fr = uniform_faces(0.1, 1.3, nr)
+    ft = uniform_faces(math.pi / 4, 3 * math.pi / 4, nt)
+    fph = uniform_faces(math.pi / 4, 3 * math.pi / 4, nph)
+    gamma = 5.0 / 3.0
+    spec = _spec("sedov_wedge_3d", 3, [nr, nt, nph], [fr, ft, fph], [BC_TRANSMISSIVE] * 3, [BC_TRANSMISSIVE] * 3, gamma,
+                 LIM_MINMOD, coords=SPHERICAL, cfl=0.6, steps=None, t_end=t_end, seed=0)
+    r, th, ph = centres(fr), centres(ft), centres(fph)
+    R, TH, PH = r[None, None, :], th[None, :, None], ph[:, None, None]
+    r0, th0, ph0 = 0.7, math.pi / 2, math.pi / 2
+    # Cartesian distance of the cell centres to the blast point
+    x, y, z = R * np.sin(TH) * np.cos(PH), R * np.sin(TH) * np.sin(PH), R * np.cos(TH) + 0.0 * PH
+    x0, y0, z0 = r0 * math.sin(th0) * math.cos(ph0), r0 * math.sin(th0) * math.sin(ph0), r0 * math.cos(th0)
+    hot = (x - x0) ** 2 + (y - y0) ** 2 + (z - z0) ** 2 < (3.5 * (fr[1] - fr[0])) ** 2
+    dV = ((fr[1:] ** 3 - fr[:-1] ** 3) / 3.0)[None, None, :] * (np.cos(ft[:-1]) - np.cos(ft[1:]))[None, :, None] \
+        * (fph[1:] - fph[:-1])[:, None, None]
+    W = np.zeros((5, nph, nt, nr))
+    W[0] = 1.0
+    W[4] = 0.01
+    W[4][hot] = (gamma - 1.0) * 1.0 / float(np.sum(dV[hot]))
+    return spec, W
+
+
 CONFIGS = {"sod_1d": sod_1d, "kh_2d": kh_2d, "sedov_3d": sedov_3d, "rt_3d": rt_3d, "wedge_3d": wedge_3d}
 
 

@@ -56,6 +56,7 @@ REDUCED = {
     "sedov_3d": lambda: wl.sedov_3d((72, 44, 38)),
     "rt_3d": lambda: wl.rt_3d((70, 36, 42)),
     "wedge_3d": lambda: wl.wedge_3d((104, 22, 26)),
+    "sedov_wedge_3d": lambda: wl.sedov_wedge_3d((72, 40, 36)),   # SURVEY 8(f) rank 3 (Sect. 4.3)
 }
 
 
@@ -255,6 +256,7 @@ FULL = {
     "sedov_3d": (lambda: wl.sedov_3d(256), "tile2_uni"),
     "rt_3d": (lambda: wl.rt_3d(512), "tile2_uni"),
     "wedge_3d": (lambda: wl.wedge_3d((1024, 256, 256)), "tile2"),
+    "sedov_wedge_3d": (lambda: wl.sedov_wedge_3d(256), "tile2"),
 }
 
 
@@ -310,6 +312,8 @@ def test_full_size_sampled_parity(hx, oxlib, name):
         extra = [(n[0] // 2 + a, n[1] // 2 + b, n[2] // 2 + c) for a in range(-5, 5) for b in (-4, -1, 0, 3) for c in (-4, 0, 3)]
     elif name == "rt_3d":       # the perturbed interface slab around z = 1
         extra = [(37 * q % n[0], 91 * q % n[1], n[2] // 2 + c) for q in range(40) for c in (-14, -2, -1, 0, 1, 13)]
+    elif name == "sedov_wedge_3d":   # the blast region around (r0, theta0, phi0) = mid-domain
+        extra = [(n[0] // 2 + a, n[1] // 2 + b, n[2] // 2 + c) for a in range(-5, 5) for b in (-4, -1, 0, 3) for c in (-4, 0, 3)]
     else:                       # the bomb in the first radial cells and the composition shell edges
         extra = [(a, 53 * a % n[1], 29 * a % n[2]) for a in list(range(0, 8)) + [161, 162, 307, 308, 471, 472, 473]]
     worst = 0.0
@@ -325,3 +329,22 @@ def test_full_size_sampled_parity(hx, oxlib, name):
         m0 = float(np.sum(o.get_state()[0], dtype=np.float64))
         m1 = float(np.sum(Ug[0], dtype=np.float64))
         assert abs(m1 - m0) <= 1e-12 * m0
+
+
+def test_step_is_deterministic(hx):
+    """Two handles, same input, five steps: bitwise identical states and time steps.  (A race in the shared-memory
+    exchange or in the in-place plane conversion would show up as run-to-run differences; compute-sanitizer is
+    not available on this pool.)"""
+    for make in (lambda: wl.rt_3d((64, 40, 36)), lambda: wl.wedge_3d((72, 24, 20))):
+        spec, W = make()
+        out = []
+        for _ in range(2):
+            g = hx.Hydro(spec)
+            g.set_state(np.ascontiguousarray(W), hx.PRIMITIVE)
+            dts = []
+            for _s in range(5):
+                dts.append(g.compute_dt(spec["cfl"]))
+                g.step(dts[-1])
+            out.append((dts, g.get_state()))
+        assert out[0][0] == out[1][0]
+        assert np.array_equal(out[0][1], out[1][1])
