@@ -24,7 +24,7 @@ typedef struct ox_handle ox_handle;
 enum { OX_OK = 0, OX_ERR_INVALID_ARG = -1, OX_ERR_ALLOC = -2, OX_ERR_NONPHYSICAL = -4, OX_ERR_UNSUPPORTED = -5 };
 enum { OX_CARTESIAN = 0, OX_SPHERICAL = 1 };
 enum { OX_BC_PERIODIC = 0, OX_BC_TRANSMISSIVE = 1, OX_BC_REFLECTING = 2, OX_BC_WEDGE = 3 };
-enum { OX_EOS_IDEAL = 0 };
+enum { OX_EOS_IDEAL = 0 /* Eq. 5 */, OX_EOS_GAS_RADIATION = 1 /* Eq. 6-7: ideal gas in equilibrium with radiation */ };
 enum { OX_RIEMANN_HLL = 0, OX_RIEMANN_HLLC = 1 };
 enum { OX_LIM_NONE = 0, OX_LIM_MINMOD = 1, OX_LIM_VANLEER = 2, OX_LIM_VANALBADA = 3, OX_LIM_MC = 4 };
 enum { OX_GRAV_NONE = 0, OX_GRAV_UNIFORM = 1, OX_GRAV_POINT_MASS = 2 };
@@ -46,6 +46,8 @@ typedef struct {
   int gravity;
   double g[3];         /* OX_GRAV_UNIFORM: acceleration vector                                  */
   double GM;           /* OX_GRAV_POINT_MASS: g = -GM/r_c^2 e_r (spherical only), Eq. 3         */
+  double eos_R;        /* OX_EOS_GAS_RADIATION: k_b / mu (gas constant per unit mass), Eq. 6a     */
+  double eos_ar;       /* OX_EOS_GAS_RADIATION: radiation constant a_r, Eq. 6a-6b                 */
 } ox_config;
 
 int ox_create(const ox_config* cfg, ox_handle** out);
@@ -67,6 +69,11 @@ int ox_cell_update(ox_handle* h, int i, int j, int k, double dt, double* out);
 int ox_riemann_flux(int riemann, double gamma, int ndim, int ns, int dir, const double* UL, const double* UR, double* F);
 /* Analytic flux F_dir(U). */
 int ox_physical_flux(double gamma, int ndim, int ns, int dir, const double* U, double* F);
+/* EOS closures for the pins: P(rho, e) (Eq. 5 / Eq. 6 through the Newton-Raphson solve for T, L102), e(rho, P),
+ * c_s(rho, P) (Eq. 5 / Eq. 7).  eos = OX_EOS_*; R = k_b/mu and ar are ignored by the ideal gas. */
+double ox_eos_pressure(int eos, double gamma, double R, double ar, double rho, double e);
+double ox_eos_energy(int eos, double gamma, double R, double ar, double rho, double P);
+double ox_eos_sound_speed(int eos, double gamma, double R, double ar, double rho, double P);
 double ox_limiter(int limiter, double a, double b);
 /* Geometry of interior or ghost cell (i,j,k): dV, dS[d][0 = minus face, 1 = plus face], centre xc[d]. */
 int ox_cell_geometry(const ox_handle* h, int i, int j, int k, double* dV, double* dS6, double* xc3);

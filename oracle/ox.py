@@ -29,6 +29,7 @@ class OxConfig(C.Structure):
         ("eos", C.c_int), ("gamma", C.c_double),
         ("riemann", C.c_int), ("limiter", C.c_int), ("n_scalars", C.c_int),
         ("gravity", C.c_int), ("g", C.c_double * 3), ("GM", C.c_double),
+        ("eos_R", C.c_double), ("eos_ar", C.c_double),
     ]
 
 
@@ -50,6 +51,9 @@ def lib():
         L.ox_step.argtypes = [vp, C.c_double]
         L.ox_cell_update.argtypes = [vp, ip, ip, ip, C.c_double, dp]
         L.ox_riemann_flux.argtypes = [ip, C.c_double, ip, ip, ip, dp, dp, dp]
+        for f in (L.ox_eos_pressure, L.ox_eos_energy, L.ox_eos_sound_speed):
+            f.argtypes = [ip] + [C.c_double] * 5
+            f.restype = C.c_double
         L.ox_physical_flux.argtypes = [C.c_double, ip, ip, ip, dp, dp]
         L.ox_limiter.argtypes = [ip, C.c_double, C.c_double]
         L.ox_limiter.restype = C.c_double
@@ -93,6 +97,9 @@ def make_config(spec: dict) -> tuple:
             cfg.spacing[d] = SPACING_CUSTOM
     cfg.eos = 0
     cfg.gamma = float(spec["gamma"])
+    cfg.eos = int(spec.get("eos", 0))
+    cfg.eos_R = float(spec.get("eos_R", 0.0))
+    cfg.eos_ar = float(spec.get("eos_ar", 0.0))
     cfg.riemann = int(spec.get("riemann", RIEMANN_HLLC))
     cfg.limiter = int(spec.get("limiter", LIM_MINMOD))
     cfg.n_scalars = int(spec.get("n_scalars", 0))
@@ -185,6 +192,21 @@ class Oracle:
         if rc != OK:
             raise OracleError(rc, "ox_faces")
         return out
+
+
+EOS_IDEAL, EOS_GAS_RADIATION = 0, 1
+
+
+def eos_pressure(eos, gamma, R, ar, rho, e):
+    return lib().ox_eos_pressure(eos, gamma, R, ar, rho, e)
+
+
+def eos_energy(eos, gamma, R, ar, rho, P):
+    return lib().ox_eos_energy(eos, gamma, R, ar, rho, P)
+
+
+def eos_sound_speed(eos, gamma, R, ar, rho, P):
+    return lib().ox_eos_sound_speed(eos, gamma, R, ar, rho, P)
 
 
 def riemann_flux(riemann, gamma, ndim, ns, direction, UL, UR):

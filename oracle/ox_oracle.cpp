@@ -123,8 +123,58 @@ double gravity(const ox_handle* h, int d, int idx) {
 // ----------------------------------------------------------------------------------------
 // Pointwise physics
 // ----------------------------------------------------------------------------------------
-// O1 (Eq. 1, Eq. 5): rho; u_d = m_d/rho; e = E - rho|u|^2/2; P = (gamma-1) e; f_s = (rho f_s)/rho
-void cons_to_prim(double gamma, int ndim, int nvar, const double* U, double* W) {
+// Equation of state.  Ideal gas (Eq. 5): P = (gamma-1) e, c_s = sqrt(gamma P / rho).  Gas + radiation (Eq. 6-7):
+//   e = rho R T / (gamma-1) + a_r T^4,   P = rho R T + a_r T^4 / 3   (R = k_b / mu),
+//   c_s^2 = [gamma/(gamma-1) + 20 alpha + 16 alpha^2] / [1/(gamma-1) + 12 alpha] * P_g / rho,  alpha = P_r / P_g;
+// "the pressure cannot be computed directly from the internal energy, so we first need to determine the
+// temperature ... using the internal energy equation 6a and a Newton-Raphson approach" (L102).  The same solve
+// gives T from P when a primitive state is turned into a conserved one.
+struct Eos {
+  int kind;
+  double gamma, R, ar;
+  Eos(double g) : kind(OX_EOS_IDEAL), gamma(g), R(0.0), ar(0.0) {}   // ideal gas from its adiabatic index
+  Eos(int k, double g, double r, double a) : kind(k), gamma(g), R(r), ar(a) {}
+};
+
+// Positive root of lin*T + quart*T^4 = rhs (lin, quart > 0).  The start min(rhs/lin, (rhs/quart)^(1/4)) lies at or
+// above the root of this convex increasing function, so Newton-Raphson descends monotonically onto it.
+double newton_T(double lin, double quart, double rhs) {
+  if (!(rhs > 0.0)) return rhs / lin;   // non-physical input: hand back a non-positive T, the caller's P > 0 check reports it
+  double T = std::min(rhs / lin, std::pow(rhs / quart, 0.25));
+  for (int it = 0; it < 200; ++it) {
+    const double T3 = T * T * T;
+    const double f = lin * T + quart * T3 * T - rhs;
+    const double dT = f / (lin + 4.0 * quart * T3);
+    T -= dT;
+    if (std::fabs(dT) <= 1e-16 * T) break;
+  }
+  return T;
+}
+
+double eos_pressure(const Eos& q, double rho, double e) {   // P(rho, e)
+  if (q.kind == OX_EOS_IDEAL) return (q.gamma - 1.0) * e;
+  const double T = newton_T(rho * q.R / (q.gamma - 1.0), q.ar, e);
+  return rho * q.R * T + q.ar * T * T * T * T / 3.0;
+}
+
+double eos_energy(const Eos& q, double rho, double P) {     // e(rho, P)
+  if (q.kind == OX_EOS_IDEAL) return P / (q.gamma - 1.0);
+  const double T = newton_T(rho * q.R, q.ar / 3.0, P);
+  return rho * q.R * T / (q.gamma - 1.0) + q.ar * T * T * T * T;
+}
+
+double eos_sound_speed(const Eos& q, double rho, double P) {   // c_s(rho, P)
+  if (q.kind == OX_EOS_IDEAL) return std::sqrt(q.gamma * P / rho);
+  const double T = newton_T(rho * q.R, q.ar / 3.0, P);
+  const double Pg = rho * q.R * T, Pr = q.ar * T * T * T * T / 3.0;
+  const double al = Pr / Pg;
+  return std::sqrt((q.gamma / (q.gamma - 1.0) + 20.0 * al + 16.0 * al * al) / (1.0 / (q.gamma - 1.0) + 12.0 * al) * Pg / rho);
+}
+
+Eos eos_of(const ox_config& c) { return Eos(c.eos, c.gamma, c.eos_R, c.eos_ar); }
+
+// O1 (Eq. 1, Eq. 5 / 6): rho; u_d = m_d/rho; e = E - rho|u|^2/2; P = P(rho, e); f_s = (rho f_s)/rho
+void cons_to_prim(const Eos& eos, int ndim, int nvar, const double* U, double* W) {
   const double rho = U[0];
   W[0] = rho;
   double u2 = 0.0;
@@ -133,11 +183,11 @@ void cons_to_prim(double gamma, int ndim, int nvar, const double* U, double* W) 
     u2 += W[1 + d] * W[1 + d];
   }
   const double e = U[1 + ndim] - 0.5 * rho * u2;
-  W[1 + ndim] = (gamma - 1.0) * e;
+  W[1 + ndim] = eos_pressure(eos, rho, e);
   for (int s = 2 + ndim; s < nvar; ++s) W[s] = U[s] / rho;
 }
 
-void prim_to_cons(double gamma, int ndim, int nvar, const double* W, double* U) {
+void prim_to_cons(const Eos& eos, int ndim, int nvar, const double* W, double* U) {
   const double rho = W[0];
   U[0] = rho;
   double u2 = 0.0;
@@ -145,15 +195,15 @@ void prim_to_cons(double gamma, int ndim, int nvar, const double* W, double* U) 
     U[1 + d] = rho * W[1 + d];
     u2 += W[1 + d] * W[1 + d];
   }
-  U[1 + ndim] = W[1 + ndim] / (gamma - 1.0) + 0.5 * rho * u2;
+  U[1 + ndim] = eos_energy(eos, rho, W[1 + ndim]) + 0.5 * rho * u2;
   for (int s = 2 + ndim; s < nvar; ++s) U[s] = rho * W[s];
 }
 
 // Analytic flux in direction dir from primitives (Eq. 1):
 // (rho u_n, rho u_n u_d + P delta_{d,dir}, (E+P) u_n, rho f_s u_n)
-void flux_from_prim(double gamma, int ndim, int nvar, int dir, const double* W, double* F) {
+void flux_from_prim(const Eos& eos, int ndim, int nvar, int dir, const double* W, double* F) {
   double U[NVMAX];
-  prim_to_cons(gamma, ndim, nvar, W, U);
+  prim_to_cons(eos, ndim, nvar, W, U);
   const double un = W[1 + dir];
   const double P = W[1 + ndim];
   F[0] = U[0] * un;
@@ -183,16 +233,16 @@ double limiter(int lim, double a, double b) {
 
 // O5 Riemann flux between conserved states UL | UR across a face normal to dir (Toro 2009,
 // ch. 10; wave-speed estimates of Davis, reading R14; ties per R15).
-void riemann_flux(int solver, double gamma, int ndim, int nvar, int dir, const double* UL, const double* UR,
+void riemann_flux(int solver, const Eos& eos, int ndim, int nvar, int dir, const double* UL, const double* UR,
                   double* F) {
   double WL[NVMAX], WR[NVMAX], FL[NVMAX], FR[NVMAX];
-  cons_to_prim(gamma, ndim, nvar, UL, WL);
-  cons_to_prim(gamma, ndim, nvar, UR, WR);
-  flux_from_prim(gamma, ndim, nvar, dir, WL, FL);
-  flux_from_prim(gamma, ndim, nvar, dir, WR, FR);
+  cons_to_prim(eos, ndim, nvar, UL, WL);
+  cons_to_prim(eos, ndim, nvar, UR, WR);
+  flux_from_prim(eos, ndim, nvar, dir, WL, FL);
+  flux_from_prim(eos, ndim, nvar, dir, WR, FR);
   const int ie = 1 + ndim;
   const double rL = WL[0], rR = WR[0], uL = WL[1 + dir], uR = WR[1 + dir], PL = WL[ie], PR = WR[ie];
-  const double cL = std::sqrt(gamma * PL / rL), cR = std::sqrt(gamma * PR / rR);
+  const double cL = eos_sound_speed(eos, rL, PL), cR = eos_sound_speed(eos, rR, PR);
   const double SL = std::min(uL - cL, uR - cR);
   const double SR = std::max(uL + cL, uR + cR);
   if (solver == OX_RIEMANN_HLL) {
@@ -279,7 +329,7 @@ void predictor(const ox_handle* h, int i, int j, int k, double dt, const double*
   const int ndim = c.ndim, nvar = h->nvar;
   const int id[3] = {i, j, k};
   double U[NVMAX];
-  prim_to_cons(c.gamma, ndim, nvar, W, U);
+  prim_to_cons(eos_of(c), ndim, nvar, W, U);
   if (c.limiter == OX_LIM_NONE) {  // R19: first-order Godunov, no predictor
     for (int d = 0; d < ndim; ++d)
       for (int v = 0; v < nvar; ++v) Um[d][v] = Up[d][v] = U[v];
@@ -302,8 +352,8 @@ void predictor(const ox_handle* h, int i, int j, int k, double dt, const double*
       Wp[d][v] = W[v] + 0.5 * del * sig;
     }
     double Fm[NVMAX], Fp[NVMAX];
-    flux_from_prim(c.gamma, ndim, nvar, d, Wm[d], Fm);
-    flux_from_prim(c.gamma, ndim, nvar, d, Wp[d], Fp);
+    flux_from_prim(eos_of(c), ndim, nvar, d, Wm[d], Fm);
+    flux_from_prim(eos_of(c), ndim, nvar, d, Wp[d], Fp);
     for (int v = 0; v < nvar; ++v) dU[v] += (Fm[v] * dS[d][0] - Fp[v] * dS[d][1]) / dV;  // O4, Eq. 18
   }
   if (c.coords == OX_SPHERICAL) {
@@ -318,8 +368,8 @@ void predictor(const ox_handle* h, int i, int j, int k, double dt, const double*
   }
   for (int v = 0; v < nvar; ++v) dU[v] *= 0.5 * dt;
   for (int d = 0; d < ndim; ++d) {
-    prim_to_cons(c.gamma, ndim, nvar, Wm[d], Um[d]);
-    prim_to_cons(c.gamma, ndim, nvar, Wp[d], Up[d]);
+    prim_to_cons(eos_of(c), ndim, nvar, Wm[d], Um[d]);
+    prim_to_cons(eos_of(c), ndim, nvar, Wp[d], Up[d]);
     for (int v = 0; v < nvar; ++v) {
       Um[d][v] += dU[v];
       Up[d][v] += dU[v];
@@ -327,7 +377,7 @@ void predictor(const ox_handle* h, int i, int j, int k, double dt, const double*
   }
   double Uc[NVMAX], Wc[NVMAX];
   for (int v = 0; v < nvar; ++v) Uc[v] = U[v] + dU[v];
-  cons_to_prim(c.gamma, ndim, nvar, Uc, Wc);
+  cons_to_prim(eos_of(c), ndim, nvar, Uc, Wc);
   Pbar = Wc[1 + ndim];
 }
 
@@ -437,7 +487,7 @@ void naive_get_U(const ox_handle* h, int i, int j, int k, double* U) {
 void naive_get_W(const ox_handle* h, int i, int j, int k, double* W) {
   double U[NVMAX];
   naive_get_U(h, i, j, k, U);
-  cons_to_prim(h->c.gamma, h->c.ndim, h->nvar, U, W);
+  cons_to_prim(eos_of(h->c), h->c.ndim, h->nvar, U, W);
 }
 
 void naive_predict(const ox_handle* h, int i, int j, int k, double dt, double Um[3][NVMAX], double Up[3][NVMAX],
@@ -461,14 +511,15 @@ void naive_face_flux(const ox_handle* h, int i, int j, int k, int d, double dt, 
   double UmL[3][NVMAX], UpL[3][NVMAX], UmR[3][NVMAX], UpR[3][NVMAX], pb;
   naive_predict(h, a[0], a[1], a[2], dt, UmL, UpL, pb);
   naive_predict(h, i, j, k, dt, UmR, UpR, pb);
-  riemann_flux(h->c.riemann, h->c.gamma, h->c.ndim, h->nvar, d, UpL[d], UmR[d], F);
+  riemann_flux(h->c.riemann, eos_of(h->c), h->c.ndim, h->nvar, d, UpL[d], UmR[d], F);
 }
 
 int check_config(const ox_config* c) {
   if (!c) return OX_ERR_INVALID_ARG;
   if (c->ndim < 1 || c->ndim > 3) return OX_ERR_INVALID_ARG;
   if (c->coords != OX_CARTESIAN && c->coords != OX_SPHERICAL) return OX_ERR_INVALID_ARG;
-  if (c->eos != OX_EOS_IDEAL) return OX_ERR_UNSUPPORTED;
+  if (c->eos != OX_EOS_IDEAL && c->eos != OX_EOS_GAS_RADIATION) return OX_ERR_UNSUPPORTED;
+  if (c->eos == OX_EOS_GAS_RADIATION && (!(c->eos_R > 0.0) || !(c->eos_ar > 0.0))) return OX_ERR_INVALID_ARG;
   if (!(c->gamma > 1.0)) return OX_ERR_INVALID_ARG;
   if (c->riemann != OX_RIEMANN_HLL && c->riemann != OX_RIEMANN_HLLC) return OX_ERR_INVALID_ARG;
   if (c->limiter < OX_LIM_NONE || c->limiter > OX_LIM_MC) return OX_ERR_INVALID_ARG;
@@ -588,7 +639,7 @@ int ox_set_state(ox_handle* h, const double* data, int form) {
         double a[NVMAX], b[NVMAX];
         for (int v = 0; v < h->nvar; ++v) a[v] = data[(size_t)v * nint + src];
         if (form == OX_PRIMITIVE) {
-          prim_to_cons(c.gamma, c.ndim, h->nvar, a, b);
+          prim_to_cons(eos_of(c), c.ndim, h->nvar, a, b);
         } else {
           for (int v = 0; v < h->nvar; ++v) b[v] = a[v];
         }
@@ -611,7 +662,7 @@ int ox_get_state(ox_handle* h, double* data, int form) {
         double a[NVMAX], b[NVMAX];
         for (int v = 0; v < h->nvar; ++v) a[v] = h->U[(size_t)v * h->ncp + src];
         if (form == OX_PRIMITIVE) {
-          cons_to_prim(c.gamma, c.ndim, h->nvar, a, b);
+          cons_to_prim(eos_of(c), c.ndim, h->nvar, a, b);
         } else {
           for (int v = 0; v < h->nvar; ++v) b[v] = a[v];
         }
@@ -634,13 +685,13 @@ int ox_compute_dt(ox_handle* h, double cfl, double* dt_out) {
         const size_t ci = h->cell(i, j, k);
         double U[NVMAX], W[NVMAX];
         for (int v = 0; v < h->nvar; ++v) U[v] = h->U[(size_t)v * h->ncp + ci];
-        cons_to_prim(c.gamma, c.ndim, h->nvar, U, W);
+        cons_to_prim(eos_of(c), c.ndim, h->nvar, U, W);
         const double rho = W[0], P = W[1 + c.ndim];
         if (!(rho > 0.0) || !(P > 0.0) || !std::isfinite(rho) || !std::isfinite(P)) {
           bad = 1;
           continue;
         }
-        const double cs = std::sqrt(c.gamma * P / rho);
+        const double cs = eos_sound_speed(eos_of(c), rho, P);
         const int id[3] = {i, j, k};
         double rate = 0.0;
         for (int d = 0; d < c.ndim; ++d) {
@@ -673,7 +724,7 @@ int ox_step(ox_handle* h, double dt) {
   for (long long ci = 0; ci < (long long)ncp; ++ci) {
     double a[NVMAX], b[NVMAX];
     for (int v = 0; v < nvar; ++v) a[v] = U[(size_t)v * ncp + ci];
-    cons_to_prim(c.gamma, ndim, nvar, a, b);
+    cons_to_prim(eos_of(c), ndim, nvar, a, b);
     for (int v = 0; v < nvar; ++v) W[(size_t)v * ncp + ci] = b[v];
   }
 
@@ -734,7 +785,7 @@ int ox_step(ox_handle* h, double dt) {
             UL[v] = Up[d][(size_t)v * ncp + cl];
             UR[v] = Um[d][(size_t)v * ncp + cr];
           }
-          riemann_flux(c.riemann, c.gamma, ndim, nvar, d, UL, UR, Fl);
+          riemann_flux(c.riemann, eos_of(c), ndim, nvar, d, UL, UR, Fl);
           for (int v = 0; v < nvar; ++v) F[d][(size_t)v * ncp + cr] = Fl[v];
         }
   }
@@ -799,6 +850,13 @@ int ox_physical_flux(double gamma, int ndim, int ns, int dir, const double* U, d
   cons_to_prim(gamma, ndim, 2 + ndim + ns, U, W);
   flux_from_prim(gamma, ndim, 2 + ndim + ns, dir, W, F);
   return OX_OK;
+}
+
+
+double ox_eos_pressure(int eos, double gamma, double R, double ar, double rho, double e) { return eos_pressure(Eos(eos, gamma, R, ar), rho, e); }
+double ox_eos_energy(int eos, double gamma, double R, double ar, double rho, double P) { return eos_energy(Eos(eos, gamma, R, ar), rho, P); }
+double ox_eos_sound_speed(int eos, double gamma, double R, double ar, double rho, double P) {
+  return eos_sound_speed(Eos(eos, gamma, R, ar), rho, P);
 }
 
 double ox_limiter(int lim, double a, double b) { return limiter(lim, a, b); }

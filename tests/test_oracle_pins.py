@@ -545,6 +545,10 @@ CASES_P11 = [
     ("s2d", 2, [6, 5], 1, [2, 3], [1, 3], 2, 2, 1, 1),
     ("s1d", 1, [8], 1, [2], [1], 2, 1, 1, 1),
     ("s3d_first_order", 3, [4, 4, 4], 1, [2, 3, 0], [1, 3, 0], 2, 0, 1, 0),
+    # gas + radiation EOS (Eq. 6-7; names ending in _rad): P_r / P_g of order 0.1-1 on these states
+    ("c3d_rad", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 2),
+    ("s3d_rad", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 2),
+    ("c1d_hll_rad", 1, [9], 0, [1], [2], 0, 2, 0, 0),
 ]
 
 
@@ -566,6 +570,8 @@ def random_problem(ox, case, seed=0):
         kw.update(gravity=ox.GRAV_UNIFORM, g=[0.3, -0.2, -0.5])
     elif grav == 2:
         kw.update(gravity=ox.GRAV_POINT_MASS, GM=0.8)
+    if name.endswith("_rad"):
+        kw.update(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0)
     spec = wl._spec(name, ndim, n, faces, bc_lo, bc_hi, 1.4, lim, **kw)
     shape = tuple((n + [1, 1])[:3][::-1])
     W = np.empty((2 + ndim + ns,) + shape)
@@ -800,3 +806,77 @@ def test_p8_offcentre_sedov_wedge_matches_similarity_solution(oxlib):
         assert abs(d - d_exact) <= 0.10 * d_exact, (d_out, d_in, d_th, d_exact)
     assert abs(d_out - d_in) <= 1.5 * dr and abs(d_out - d_th) <= 1.5 * dr, (d_out, d_in, d_th)
     assert np.max(line) > 1.6 and np.min(line) < 0.1     # a shell around an evacuated interior
+
+
+# ------------------------------------------------------------------------------------------ P12: gas + radiation EOS
+def test_p12_gas_radiation_eos_closed_forms(oxlib):
+    """Eq. 6-7 (L88-L102).  Round trip e(rho, P(rho, e)) through the Newton-Raphson solve over twelve decades of
+    P_r / P_g; the two limits (a_r -> 0: ideal gas with gamma; k_b/mu -> 0: P = e / 3, c_s^2 = (4/3) P / rho); and
+    Eq. 7 against the definition c_s^2 = (dP/drho) at constant entropy, evaluated by a symmetric difference along
+    the adiabat d(e/rho) = (P / rho^2) drho (catches a wrong coefficient in Eq. 7 as extracted)."""
+    ox = oxlib
+    GR, g, R = ox.EOS_GAS_RADIATION, 5.0 / 3.0, 1.3
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        rho, T = 10.0 ** rng.uniform(-6, 2), 10.0 ** rng.uniform(-3, 3)
+        ar = 10.0 ** rng.uniform(-3, 3)
+        P = rho * R * T + ar * T ** 4 / 3.0
+        e = rho * R * T / (g - 1.0) + ar * T ** 4                                    # Eq. 6a, 6b written out
+        assert ox.eos_energy(GR, g, R, ar, rho, P) == pytest.approx(e, rel=1e-13)
+        assert ox.eos_pressure(GR, g, R, ar, rho, e) == pytest.approx(P, rel=1e-13)
+        al = (ar * T ** 4 / 3.0) / (rho * R * T)
+        c2 = (g / (g - 1.0) + 20.0 * al + 16.0 * al * al) / (1.0 / (g - 1.0) + 12.0 * al) * R * T   # Eq. 7, P_g / rho = R T
+        assert ox.eos_sound_speed(GR, g, R, ar, rho, P) == pytest.approx(math.sqrt(c2), rel=1e-13)
+        # thermodynamic definition, symmetric difference along the adiabat
+        eps = 1e-5
+        es = e / rho
+        Pp = ox.eos_pressure(GR, g, R, ar, rho * (1 + eps), (es + P / rho ** 2 * rho * eps) * rho * (1 + eps))
+        Pm = ox.eos_pressure(GR, g, R, ar, rho * (1 - eps), (es - P / rho ** 2 * rho * eps) * rho * (1 - eps))
+        assert (Pp - Pm) / (2 * eps * rho) == pytest.approx(c2, rel=2e-6)
+    # limits
+    assert ox.eos_pressure(GR, g, R, 1e-60, 2.0, 3.0) == pytest.approx((g - 1.0) * 3.0, rel=1e-14)
+    assert ox.eos_sound_speed(GR, g, R, 1e-60, 2.0, 3.0) == pytest.approx(math.sqrt(g * 3.0 / 2.0), rel=1e-14)
+    assert ox.eos_pressure(GR, g, 1e-60, 0.7, 2.0, 3.0) == pytest.approx(1.0, rel=1e-14)
+    assert ox.eos_sound_speed(GR, g, 1e-60, 0.7, 2.0, 3.0) == pytest.approx(math.sqrt(4.0 / 3.0 * 3.0 / 2.0), rel=1e-12)
+
+
+@pytest.mark.parametrize("limit", ["gas", "radiation"])
+def test_p12_gas_radiation_limits_reduce_to_ideal_gases(oxlib, limit):
+    """The whole step with the gas + radiation EOS equals the ideal-gas step with gamma (a_r -> 0) and with 4/3
+    (k_b / mu -> 0) on a random 3-D problem with gravity, reflecting and periodic faces, two scalars."""
+    ox = oxlib
+    case = ("c3d_mixed", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 2)
+    spec, W = random_problem(ox, case)
+    ideal, rad = dict(spec), dict(spec)
+    if limit == "gas":
+        rad.update(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=1e-60)
+    else:
+        ideal["gamma"] = 4.0 / 3.0
+        rad.update(eos=wl.EOS_GAS_RADIATION, eos_R=1e-60, eos_ar=1.0)
+    a, b = make(ox, ideal, W), make(ox, rad, W)
+    for _ in range(3):
+        dt = a.compute_dt(0.4)
+        assert b.compute_dt(0.4) == pytest.approx(dt, rel=1e-12)
+        a.step(dt)
+        b.step(dt)
+    Ua, Ub = a.get_state(), b.get_state()
+    assert np.max(np.abs(Ua - Ub)) <= 1e-12 * np.max(np.abs(Ua))
+
+
+def test_p12_gas_radiation_conserves_and_keeps_uniform_states(oxlib):
+    ox = oxlib
+    spec, W = wl.smooth_periodic(3, [10, 8, 6], seed=3, n_scalars=1, limiter=wl.LIM_VANLEER)
+    spec = dict(spec, eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0)
+    o = make(ox, spec, W)
+    U0 = o.get_state()
+    run_steps(o, 0.4, 20)
+    U1 = o.get_state()
+    for v in range(U0.shape[0]):
+        assert abs(fsum(U1[v]) - fsum(U0[v])) <= 1e-13 * max(fsum(np.abs(U0[v])), 1.0)
+    Wu = np.empty_like(W)
+    for v, val in enumerate([1.3, 0.2, -0.4, 0.1, 0.9, 0.35]):
+        Wu[v] = val
+    o = make(ox, spec, Wu)
+    Ua = o.get_state()
+    run_steps(o, 0.4, 5)
+    assert np.max(np.abs(o.get_state() - Ua)) <= 1e-14 * np.max(np.abs(Ua))
