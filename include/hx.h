@@ -32,7 +32,7 @@ enum { HX_CARTESIAN = 0, HX_SPHERICAL = 1 };
 /* Boundary conditions (periodic, null gradient, reflective).  HX_BC_WEDGE is the
  * reflective condition on the angular faces of a spherical wedge (L424). */
 enum { HX_BC_PERIODIC = 0, HX_BC_TRANSMISSIVE = 1, HX_BC_REFLECTING = 2, HX_BC_WEDGE = 3 };
-enum { HX_EOS_IDEAL = 0 };                              /* Eq. 5 */
+enum { HX_EOS_IDEAL = 0 /* Eq. 5 */, HX_EOS_GAS_RADIATION = 1 /* Eq. 6-7: ideal gas in equilibrium with radiation */ };
 enum { HX_RIEMANN_HLL = 0, HX_RIEMANN_HLLC = 1 };       /* L201 */
 /* Slope limiters (L189) + first order (HX_LIM_NONE) + monotonised central (BASELINE.json configs) */
 enum { HX_LIM_NONE = 0, HX_LIM_MINMOD = 1, HX_LIM_VANLEER = 2, HX_LIM_VANALBADA = 3, HX_LIM_MC = 4 };
@@ -57,12 +57,14 @@ typedef struct {
   const double* faces[3]; /* HX_SPACING_CUSTOM: n[d]+1 strictly increasing HOST face coordinates,    */
                           /* copied during hx_create                                                 */
   int bc_lo[3], bc_hi[3]; /* periodic must be set on both sides of a direction                       */
-  int eos;                /* HX_EOS_IDEAL                                                            */
+  int eos;                /* HX_EOS_IDEAL or HX_EOS_GAS_RADIATION (T from e by Newton-Raphson, L102)         */
   double gamma;           /* adiabatic index > 1                                                     */
   int riemann, limiter, n_scalars;
   int gravity;            /* HX_GRAV_*; point mass needs HX_SPHERICAL                                */
   double g[3];            /* uniform: acceleration vector (force = +rho*g, R12)            */
   double GM;              /* point mass: g = -GM/r_c^2 e_r                                           */
+  double eos_R;           /* HX_EOS_GAS_RADIATION: k_b / mu, gas constant per unit mass (Eq. 6a); > 0         */
+  double eos_ar;          /* HX_EOS_GAS_RADIATION: radiation constant a_r (Eq. 6a-6b); > 0                    */
 } hx_config;
 
 /* Validate cfg, allocate the padded double-buffered state and the geometry tables on the current

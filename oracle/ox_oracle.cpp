@@ -141,12 +141,14 @@ struct Eos {
 double newton_T(double lin, double quart, double rhs) {
   if (!(rhs > 0.0)) return rhs / lin;   // non-physical input: hand back a non-positive T, the caller's P > 0 check reports it
   double T = std::min(rhs / lin, std::pow(rhs / quart, 0.25));
-  for (int it = 0; it < 200; ++it) {
+  // stop when the correction is a few ulp (reading R27; a bound below the rounding unit would never be met and
+  // the loop would always run to its cap); the iteration converges quadratically, ~5-9 steps (L102: "approximately ten")
+  for (int it = 0; it < 60; ++it) {
     const double T3 = T * T * T;
     const double f = lin * T + quart * T3 * T - rhs;
     const double dT = f / (lin + 4.0 * quart * T3);
     T -= dT;
-    if (std::fabs(dT) <= 1e-16 * T) break;
+    if (std::fabs(dT) <= 1e-15 * T) break;
   }
   return T;
 }

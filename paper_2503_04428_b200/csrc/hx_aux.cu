@@ -178,12 +178,12 @@ __global__ void rate_kernel(Layout L, Tables T, Phys P, const double* __restrict
       u[d] = U[(1 + d) * L.sv + o] * ir;
       u2 += u[d] * u[d];
     }
-    const double p = P.gm1 * (U[(1 + ND) * L.sv + o] - 0.5 * rho * u2);
+    const double p = eos_pressure(P, rho, U[(1 + ND) * L.sv + o] - 0.5 * rho * u2);
     if (!(rho > 0.0) || !(p > 0.0) || !isfinite(rho) || !isfinite(p)) {
       bad = true;
       continue;
     }
-    const double cs = sqrt(P.gamma * p * ir);
+    const double cs = eos_sound_speed(P, rho, p);
     double rate = 0.0;
 #pragma unroll
     for (int d = 0; d < ND; ++d) rate += (fabs(u[d]) + cs) * (T.lf[d][0][pi] * T.lf[d][1][pj] * T.lf[d][2][pk]);

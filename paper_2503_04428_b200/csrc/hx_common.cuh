@@ -48,6 +48,8 @@ struct Tables {
 struct Phys {
   double gamma, gm1, igm1;
   int limiter, riemann, gravity, spherical;
+  int eos;                // HX_EOS_IDEAL or HX_EOS_GAS_RADIATION
+  double rgas, arad;      // gas + radiation: k_b / mu and the radiation constant a_r (Eq. 6a-6b)
 };
 
 struct StepArgs {
@@ -80,7 +82,48 @@ __device__ __forceinline__ double limited_slope(int lim, double a, double b) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// cons <-> prim (Eq. 1, Eq. 5).  Field order: rho, m_d / u_d (ND of them), E / P, scalars.
+// Equation of state.  Ideal gas: Eq. 5.  Ideal gas in equilibrium with radiation (Eq. 6-7):
+//   e = rho (k_b/mu) T / (gamma-1) + a_r T^4,   P = rho (k_b/mu) T + a_r T^4 / 3,   alpha = P_r / P_g,
+//   c_s^2 = (gamma/(gamma-1) + 20 alpha + 16 alpha^2) / (1/(gamma-1) + 12 alpha) * P_g / rho.
+// T comes from e (or from P) by Newton-Raphson, as the paper prescribes; started at the smaller of the two
+// single-term roots the iterate can only move down towards the root; it stops when the correction is a few ulp.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double temperature_root(double a1, double a4, double b) {   // a1 T + a4 T^4 = b
+  if (!(b > 0.0)) return b / a1;                       // non-physical: a non-positive T makes the caller's P <= 0
+  double T = fmin(b / a1, sqrt(sqrt(b / a4)));
+  for (int it = 0; it < 60; ++it) {                    // R27: until the correction is a few ulp; quadratic, ~5-9 steps
+    const double T3 = T * T * T;
+    const double step = (fma(a4 * T3, T, a1 * T) - b) / fma(4.0 * a4, T3, a1);
+    T -= step;
+    if (fabs(step) <= 1e-15 * T) break;
+  }
+  return T;
+}
+
+__device__ __forceinline__ double eos_pressure(const Phys& P, double rho, double e) {
+  if (P.eos == HX_EOS_IDEAL) return P.gm1 * e;
+  const double T = temperature_root(rho * P.rgas * P.igm1, P.arad, e);
+  const double T2 = T * T;
+  return fma(P.arad * (1.0 / 3.0), T2 * T2, rho * P.rgas * T);
+}
+
+__device__ __forceinline__ double eos_energy(const Phys& P, double rho, double p) {
+  if (P.eos == HX_EOS_IDEAL) return p * P.igm1;
+  const double T = temperature_root(rho * P.rgas, P.arad * (1.0 / 3.0), p);
+  const double T2 = T * T;
+  return fma(P.arad, T2 * T2, rho * P.rgas * T * P.igm1);
+}
+
+__device__ __forceinline__ double eos_sound_speed(const Phys& P, double rho, double p) {
+  if (P.eos == HX_EOS_IDEAL) return sqrt(P.gamma * p / rho);
+  const double T = temperature_root(rho * P.rgas, P.arad * (1.0 / 3.0), p);
+  const double T2 = T * T;
+  const double pg = rho * P.rgas * T, al = P.arad * (1.0 / 3.0) * T2 * T2 / pg;
+  return sqrt((P.gamma * P.igm1 + al * (20.0 + 16.0 * al)) / (P.igm1 + 12.0 * al) * pg / rho);
+}
+
+// ---------------------------------------------------------------------------------------------
+// cons <-> prim (Eq. 1, Eq. 5 / 6).  Field order: rho, m_d / u_d (ND of them), E / P, scalars.
 // ---------------------------------------------------------------------------------------------
 template <int ND>
 __device__ __forceinline__ void cons_to_prim(const Phys& P, int nv, const double* U, double* W) {
@@ -93,7 +136,7 @@ __device__ __forceinline__ void cons_to_prim(const Phys& P, int nv, const double
     W[1 + d] = U[1 + d] * ir;
     u2 += W[1 + d] * W[1 + d];
   }
-  W[1 + ND] = P.gm1 * (U[1 + ND] - 0.5 * rho * u2);
+  W[1 + ND] = eos_pressure(P, rho, U[1 + ND] - 0.5 * rho * u2);
   for (int s = 2 + ND; s < nv; ++s) W[s] = U[s] * ir;
 }
 
@@ -107,7 +150,7 @@ __device__ __forceinline__ void prim_to_cons(const Phys& P, int nv, const double
     U[1 + d] = rho * W[1 + d];
     u2 += W[1 + d] * W[1 + d];
   }
-  U[1 + ND] = W[1 + ND] * P.igm1 + 0.5 * rho * u2;
+  U[1 + ND] = eos_energy(P, rho, W[1 + ND]) + 0.5 * rho * u2;
   for (int s = 2 + ND; s < nv; ++s) U[s] = rho * W[s];
 }
 
@@ -135,7 +178,7 @@ __device__ __forceinline__ void riemann_flux(const Phys& P, int nv, int dir, con
   flux_along<ND>(nv, dir, WL, UL, FL);
   flux_along<ND>(nv, dir, WR, UR, FR);
   const double rL = WL[0], rR = WR[0], uL = WL[1 + dir], uR = WR[1 + dir], pL = WL[1 + ND], pR = WR[1 + ND];
-  const double cL = sqrt(P.gamma * pL / rL), cR = sqrt(P.gamma * pR / rR);
+  const double cL = eos_sound_speed(P, rL, pL), cR = eos_sound_speed(P, rR, pR);
   const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
   if (P.riemann == HX_RIEMANN_HLL) {
     if (SL >= 0.0) {

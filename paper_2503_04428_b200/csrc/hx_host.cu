@@ -80,7 +80,8 @@ const char* check_config(const hx_config* c, int* code) {
   if (!c) return "null config";
   if (c->ndim < 1 || c->ndim > 3) return "ndim must be 1, 2 or 3";
   if (c->coords != HX_CARTESIAN && c->coords != HX_SPHERICAL) return "unknown coordinate system";
-  if (c->eos != HX_EOS_IDEAL) { *code = HX_ERR_UNSUPPORTED; return "only the ideal-gas EOS is implemented"; }
+  if (c->eos != HX_EOS_IDEAL && c->eos != HX_EOS_GAS_RADIATION) { *code = HX_ERR_UNSUPPORTED; return "unknown equation of state"; }
+  if (c->eos == HX_EOS_GAS_RADIATION && (!(c->eos_R > 0.0) || !(c->eos_ar > 0.0))) return "gas + radiation EOS needs eos_R > 0 and eos_ar > 0";
   if (!(c->gamma > 1.0)) return "gamma must be > 1";
   if (c->riemann != HX_RIEMANN_HLL && c->riemann != HX_RIEMANN_HLLC) return "unknown Riemann solver";
   if (c->limiter < HX_LIM_NONE || c->limiter > HX_LIM_MC) return "unknown limiter";
@@ -346,6 +347,9 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
   h->P.riemann = cfg->riemann;
   h->P.gravity = cfg->gravity;
   h->P.spherical = cfg->coords == HX_SPHERICAL;
+  h->P.eos = cfg->eos;
+  h->P.rgas = cfg->eos_R;
+  h->P.arad = cfg->eos_ar;
 
   const size_t bytes = (size_t)L.nvar * (size_t)L.sv * sizeof(double);
   cudaError_t e;

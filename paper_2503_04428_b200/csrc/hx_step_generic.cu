@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(128) step_generic_kernel(StepArgs a) {
     if (!(rho > 0.0) || !(p > 0.0) || !isfinite(rho) || !isfinite(p)) {
       atomicOr(a.status, 1);
     } else {
-      const double cs = sqrt(a.P.gamma * p / rho);
+      const double cs = eos_sound_speed(a.P, rho, p);
 #pragma unroll
       for (int d = 0; d < ND; ++d) {
         const double il = a.T.lf[d][0][pidx[0]] * a.T.lf[d][1][pidx[1]] * a.T.lf[d][2][pidx[2]];

@@ -15,7 +15,7 @@ from . import build as _build
 OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_NONPHYSICAL, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 CARTESIAN, SPHERICAL = 0, 1
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTING, BC_WEDGE = 0, 1, 2, 3
-EOS_IDEAL = 0
+EOS_IDEAL, EOS_GAS_RADIATION = 0, 1
 RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 LIM_NONE, LIM_MINMOD, LIM_VANLEER, LIM_VANALBADA, LIM_MC = 0, 1, 2, 3, 4
 GRAV_NONE, GRAV_UNIFORM, GRAV_POINT_MASS = 0, 1, 2
@@ -39,6 +39,7 @@ class HxConfig(C.Structure):
         ("eos", C.c_int), ("gamma", C.c_double),
         ("riemann", C.c_int), ("limiter", C.c_int), ("n_scalars", C.c_int),
         ("gravity", C.c_int), ("g", C.c_double * 3), ("GM", C.c_double),
+        ("eos_R", C.c_double), ("eos_ar", C.c_double),
     ]
 
 
@@ -107,7 +108,9 @@ def make_config(spec: dict):
             keep.append(arr)
             cfg.faces[d] = arr.ctypes.data_as(C.POINTER(C.c_double))
             cfg.spacing[d] = SPACING_CUSTOM
-    cfg.eos = EOS_IDEAL
+    cfg.eos = int(spec.get("eos", EOS_IDEAL))
+    cfg.eos_R = float(spec.get("eos_R", 0.0))
+    cfg.eos_ar = float(spec.get("eos_ar", 0.0))
     cfg.gamma = float(spec["gamma"])
     cfg.riemann = int(spec.get("riemann", RIEMANN_HLLC))
     cfg.limiter = int(spec.get("limiter", LIM_MINMOD))

@@ -219,6 +219,16 @@ def sedov_wedge_3d(n=256, t_end=0.08):
     return spec, W
 
 
+def wedge_3d_rad(n=(1024, 256, 256), seed=1005):
+    """the C5 wedge with the paper's production EOS for stellar explosions, an ideal gas in
+    equilibrium with radiation (Eq. 6-7, used for the supernova runs, L377).  Same primitive
+    fields (rho, u, P, f) as wedge_3d; gas gamma = 5/3, k_b/mu = 1, a_r = 30 in code units: P_r/P_g is 0.02-0.15 in the
+    envelope (gas dominated, both terms matter) and about 16 in the bomb (radiation dominated)."""
+    spec, W = wedge_3d(n, seed)
+    spec = dict(spec, name="wedge_3d_rad", gamma=5.0 / 3.0, eos=EOS_GAS_RADIATION, eos_R=1.0, eos_ar=30.0)
+    return spec, W
+
+
 CONFIGS = {"sod_1d": sod_1d, "kh_2d": kh_2d, "sedov_3d": sedov_3d, "rt_3d": rt_3d, "wedge_3d": wedge_3d}
 
 

@@ -28,9 +28,10 @@ def test_library_loads_and_exports_every_declared_symbol():
 
 
 def test_config_struct_matches_header_layout():
-    # 3 ints, 6 doubles, 3 ints, 3 pointers, 6 ints, int + double, 3 ints, int, 3 doubles, double
-    assert C.sizeof(hx.HxConfig) == 200
+    # 3 ints, 6 doubles, 3 ints, 3 pointers, 6 ints, int + double, 3 ints, int, 3 doubles, double, 2 doubles (EOS constants)
+    assert C.sizeof(hx.HxConfig) == 216
     assert hx.HxConfig.faces.offset == 88 and hx.HxConfig.gamma.offset == 144 and hx.HxConfig.GM.offset == 192
+    assert hx.HxConfig.eos_R.offset == 200 and hx.HxConfig.eos_ar.offset == 208
 
 
 def test_invalid_arguments_rejected_without_gpu():
@@ -38,12 +39,15 @@ def test_invalid_arguments_rejected_without_gpu():
     out = C.c_void_p()
     assert L.hx_create(None, C.byref(out)) == hx.ERR_INVALID_ARG
     spec, _ = wl.sod_1d(16)
-    for key, val in (("gamma", 1.0), ("ndim", 4), ("limiter", 9), ("riemann", 5), ("n_scalars", 40)):
+    for key, val in (("gamma", 1.0), ("ndim", 4), ("limiter", 9), ("riemann", 5), ("n_scalars", 40), ("eos", 1)):   # eos 1 (gas + radiation) without its constants
         bad = dict(spec)
         bad[key] = val
         cfg, keep = hx.make_config(bad)
         assert L.hx_create(C.byref(cfg), C.byref(out)) == hx.ERR_INVALID_ARG, key
         assert not out.value
+    bad = dict(spec, eos=2)                          # unknown equation of state
+    cfg, keep = hx.make_config(bad)
+    assert L.hx_create(C.byref(cfg), C.byref(out)) == hx.ERR_UNSUPPORTED
     bad = dict(spec)
     bad["bc_lo"] = [hx.BC_PERIODIC, 0, 0]          # periodic on one side only
     cfg, keep = hx.make_config(bad)

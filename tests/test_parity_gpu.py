@@ -57,6 +57,7 @@ REDUCED = {
     "rt_3d": lambda: wl.rt_3d((70, 36, 42)),
     "wedge_3d": lambda: wl.wedge_3d((104, 22, 26)),
     "sedov_wedge_3d": lambda: wl.sedov_wedge_3d((72, 40, 36)),   # SURVEY 8(f) rank 3 (Sect. 4.3)
+    "wedge_3d_rad": lambda: wl.wedge_3d_rad((72, 18, 20)),        # SURVEY 8(f) rank 1 (gas + radiation EOS, Eq. 6-7)
 }
 
 
