@@ -53,7 +53,7 @@ def alg_flops_per_cell(spec):
     """Algorithmic fp64 flops per 3-D cell-update (hand count from O1-O7 with every
     predictor and face flux computed once; + and x count 1 each, so an FMA is 2; div and sqrt 1 each):
     629 for nvar = 5, HLLC/HLL + minmod; +4 per slope for MC / van Leer, +6 van Albada; +84 per passive
-    scalar; +31 gravity; +65 spherical sources."""
+    scalar; +31 gravity; +65 spherical sources; +1025 for the gas + radiation EOS (Newton solves for T)."""
     ns = spec["nvar"] - 2 - spec["ndim"]
     nvar = spec["nvar"]
     lim_extra = {wl.LIM_NONE: -1, wl.LIM_MINMOD: 0, wl.LIM_VANLEER: 4, wl.LIM_VANALBADA: 6, wl.LIM_MC: 4}[spec["limiter"]]
@@ -62,6 +62,10 @@ def alg_flops_per_cell(spec):
         f += 31
     if spec["coords"] == wl.SPHERICAL:
         f += 65
+    if spec.get("eos", 0) == wl.EOS_GAS_RADIATION:
+        # Eq. 6-7: 15 Newton-Raphson solves for T per cell-update (cons->prim, 6 face states P->e, 6 predicted states
+        # e->P, U^n, CFL rate), about 7 iterations of 9 flop (+, x, one division) each; Eq. 7 adds ~10 per sound speed
+        f += 15 * 7 * 9 + 8 * 10
     return f
 
 

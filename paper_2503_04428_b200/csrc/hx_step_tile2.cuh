@@ -188,17 +188,53 @@ __device__ __forceinline__ void tma_load_plane(const CUtensorMap* tmap, void* ds
 }
 
 // ------------------------------------------------------------------------------------------------
+// Gas + radiation EOS (Eq. 6-7; EOS == HX_EOS_GAS_RADIATION instantiations).  T is the positive root of
+// a1 T + a4 T^4 = b, by Newton-Raphson as the paper prescribes (L102), from the smaller single-term root (the
+// iterate then only moves down), until the correction is a few ulp (R27); reciprocals by seed + cubic correction.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double gr_temperature(double a1, double a4, double b) {
+  if (!(b > 0.0)) return b * rcp3(a1);                    // non-physical: T <= 0, hence P <= 0, which the rate check reports
+  double T = dmin(b * rcp3(a1), sqrt3(sqrt3(b * rcp3(a4))));
+  for (int it = 0; it < 60; ++it) {
+    const double T3 = T * T * T;
+    const double step = (fma(a4 * T3, T, a1 * T) - b) * rcp3(fma(4.0 * a4, T3, a1));
+    T -= step;
+    if (fabs(step) <= 1e-15 * T) break;
+  }
+  return T;
+}
+// P and c_s from (rho, 1/rho, e); e from (rho, P)
+__device__ __forceinline__ void gr_from_energy(const Phys& P, double rho, double ir, double e, double& p, double& c) {
+  const double T = gr_temperature(rho * P.rgas * P.igm1, P.arad, e);
+  const double T3 = T * T * T;
+  const double pg = rho * P.rgas * T;
+  p = fma(P.arad * (1.0 / 3.0) * T3, T, pg);
+  const double al = P.arad * (1.0 / 3.0) * T3 * ir * rcp3(P.rgas);   // P_r / P_g
+  c = sqrt3(fma(al, fma(16.0, al, 20.0), P.gamma * P.igm1) * rcp3(fma(12.0, al, P.igm1)) * P.rgas * T);
+}
+__device__ __forceinline__ double gr_energy(const Phys& P, double rho, double p) {
+  const double T = gr_temperature(rho * P.rgas, P.arad * (1.0 / 3.0), p);
+  const double T2 = T * T;
+  return fma(P.arad, T2 * T2, rho * P.rgas * T * P.igm1);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Pointwise pieces of the scheme.  Field order of W / U: rho, u|m [3], P|E, scalars f|rho f.
 // ------------------------------------------------------------------------------------------------
-template <int NV>
-__device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, double* W) {   // Eq. 1, Eq. 5
+template <int NV, int EOS = HX_EOS_IDEAL>
+__device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, double* W) {   // Eq. 1, Eq. 5 / 6
   const double ir = rcp3(U[0]);
   W[0] = U[0];
   W[1] = U[1] * ir;
   W[2] = U[2] * ir;
   W[3] = U[3] * ir;
   const double ke2 = fma(U[3], W[3], fma(U[2], W[2], U[1] * W[1]));
-  W[4] = P.gm1 * fma(-0.5, ke2, U[4]);
+  if (EOS == HX_EOS_IDEAL) {
+    W[4] = P.gm1 * fma(-0.5, ke2, U[4]);
+  } else {
+    double c;
+    gr_from_energy(P, U[0], ir, fma(-0.5, ke2, U[4]), W[4], c);
+  }
 #pragma unroll
   for (int s = 5; s < NV; ++s) W[s] = U[s] * ir;
 }
@@ -206,7 +242,7 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
 // One face of the cell along DIR: face primitives Wc + sc t (Eq. 17; sc = -+1, or -+hw*idx on uniform grids), their conserved form Uf, and the
 // analytic flux of that state accumulated into the half-step increment dU with the signed, (dt/2)-scaled
 // area/volume coefficient `coef` (Eq. 18: + for the lower face, - for the upper face).
-template <int NV, int DIR>
+template <int NV, int DIR, int EOS = HX_EOS_IDEAL>
 __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double sc, double coef, double* Uf, double* dU,
                                                double* unc_out = nullptr) {
   double Wf[NV];
@@ -218,7 +254,7 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
   Uf[2] = r * Wf[2];
   Uf[3] = r * Wf[3];
   const double ke2 = fma(Uf[3], Wf[3], fma(Uf[2], Wf[2], Uf[1] * Wf[1]));
-  Uf[4] = fma(0.5, ke2, Wf[4] * P.igm1);
+  Uf[4] = fma(0.5, ke2, EOS == HX_EOS_IDEAL ? Wf[4] * P.igm1 : gr_energy(P, r, Wf[4]));
   const double unc = Wf[1 + DIR] * coef;
   if (unc_out) *unc_out = unc;   // signed (dt/2) dS/dV u_n of this face: what a passive scalar's flux rides on
   dU[0] = fma(r, unc, dU[0]);
@@ -236,7 +272,7 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
 
 // Predicted face state U^{n+1/2} = cons(Wf) + dU (Eq. 18) as the record the Riemann solver consumes:
 // q = rho, u[3], P, E, c_s, scalars f.
-template <int NV>
+template <int NV, int EOS = HX_EOS_IDEAL>
 __device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, const double* dU, double* q) {
   const double r = Uf[0] + dU[0];
   const double m1 = Uf[1] + dU[1], m2 = Uf[2] + dU[2], m3 = Uf[3] + dU[3];
@@ -248,9 +284,13 @@ __device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, cons
   q[1] = m1 * ir;
   q[2] = m2 * ir;
   q[3] = m3 * ir;
-  q[4] = P.gm1 * e;
   q[5] = E;
-  q[6] = sqrt3((P.gamma * P.gm1) * ir * e);              // c^2 = gamma P / rho
+  if (EOS == HX_EOS_IDEAL) {
+    q[4] = P.gm1 * e;
+    q[6] = sqrt3((P.gamma * P.gm1) * ir * e);            // c^2 = gamma P / rho
+  } else {
+    gr_from_energy(P, r, ir, e, q[4], q[6]);
+  }
 #pragma unroll
   for (int s = 5; s < NV; ++s) q[2 + s] = (Uf[s] + dU[s]) * ir;
 }
@@ -349,7 +389,7 @@ __device__ __forceinline__ void sqrt3_n(const double* x, double* y) {
 }
 
 // N predicted face states at once (same arithmetic as pred_state)
-template <int NV, int N>
+template <int NV, int N, int EOS = HX_EOS_IDEAL>
 __device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q, double* const* ir_out = nullptr) {
   double r[N], m1[N], m2[N], m3[N], E[N], mm[N], ir[N], e[N], x[N], c[N];
 #pragma unroll
@@ -369,16 +409,24 @@ __device__ __forceinline__ void pred_states(const Phys& P, const double* const* 
   for (int k = 0; k < N; ++k) mm[k] = fma(m3[k], m3[k], mm[k]);
 #pragma unroll
   for (int k = 0; k < N; ++k) e[k] = fma(-0.5 * ir[k], mm[k], E[k]);
+  double pr[N];
+  if (EOS == HX_EOS_IDEAL) {
 #pragma unroll
-  for (int k = 0; k < N; ++k) x[k] = (P.gamma * P.gm1) * ir[k] * e[k];
-  sqrt3_n<N>(x, c);
+    for (int k = 0; k < N; ++k) x[k] = (P.gamma * P.gm1) * ir[k] * e[k];
+    sqrt3_n<N>(x, c);
+#pragma unroll
+    for (int k = 0; k < N; ++k) pr[k] = P.gm1 * e[k];
+  } else {
+#pragma unroll
+    for (int k = 0; k < N; ++k) gr_from_energy(P, r[k], ir[k], e[k], pr[k], c[k]);
+  }
 #pragma unroll
   for (int k = 0; k < N; ++k) {
     q[k][0] = r[k];
     q[k][1] = m1[k] * ir[k];
     q[k][2] = m2[k] * ir[k];
     q[k][3] = m3[k] * ir[k];
-    q[k][4] = P.gm1 * e[k];
+    q[k][4] = pr[k];
     q[k][5] = E[k];
     q[k][6] = c[k];
     if (ir_out) *ir_out[k] = ir[k];
@@ -471,11 +519,12 @@ __device__ __forceinline__ void hllc_n(const int (&dir)[N], const double* const*
 // setmaxnreg: the ring path needs far fewer registers than it is given at launch, and ptxas interleaves the
 // independent fp64 chains of the owner path only when it has ~200 registers (at 168 it emits them serially).
 // ------------------------------------------------------------------------------------------------
-template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int TY>
+template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int TY, int EOS = HX_EOS_IDEAL>
 __global__ void __launch_bounds__((TY + 4) * 32, 1)
 step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Args a) {
   static_assert(TY % 4 == 0 && TY >= 4 && TY <= 32, "owner warps must fill whole warpgroups (setmaxnreg)");
   static_assert(!(UNI && SPH), "UNI is for Cartesian grids");
+  static_assert(EOS == HX_EOS_IDEAL || EOS == HX_EOS_GAS_RADIATION, "unknown equation of state");
   using SM = Smem<NV, TY>;
   constexpr int NF = SM::NF, FSTR = SM::FSTR, XSTR = SM::XSTR, YSTR = SM::YSTR, XP = SM::XP;
   constexpr int PSTR = (int)(SM::plane_stride / sizeof(double));
@@ -607,7 +656,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     double U[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) U[v] = pl[v * FSTR + off];
-    prim_of_cons<NV>(P, U, Wout);
+    prim_of_cons<NV, EOS>(P, U, Wout);
     if (store) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) pl[v * FSTR + off] = Wout[v];
@@ -661,7 +710,13 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     const double mm = fma(Ul[3], Ul[3], fma(Ul[2], Ul[2], Ul[1] * Ul[1]));
     const double ir = rcp3(Ul[0]);
     const double e = fma(-0.5 * ir, mm, Ul[4]);
-    const double cs = sqrt3((P.gamma * P.gm1) * ir * e);
+    double cs;
+    if (EOS == HX_EOS_IDEAL) {
+      cs = sqrt3((P.gamma * P.gm1) * ir * e);
+    } else {
+      double pn;
+      gr_from_energy(P, Ul[0], ir, e, pn, cs);           // e <= 0 gives T <= 0 and a NaN sound speed, like the ideal branch
+    }
     const double il2 = UNI ? a.uil[2] : il2xy * ZT(5, max(pkc, zb));
     const double rate = fma(fma(fabs(Ul[1]), ir, cs), il0, fma(fma(fabs(Ul[2]), ir, cs), il1, fma(fabs(Ul[3]), ir, cs) * il2));
     const bool fine = (Ul[0] > 0.0) && (rate < __longlong_as_double(0x7ff0000000000000LL));
@@ -698,23 +753,23 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
     }
-    face_cons_flux<NVP, 0>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU, unc6 ? unc6 + 0 : nullptr);
-    face_cons_flux<NVP, 0>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU, unc6 ? unc6 + 1 : nullptr);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU, unc6 ? unc6 + 0 : nullptr);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU, unc6 ? unc6 + 1 : nullptr);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
     }
-    face_cons_flux<NVP, 1>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU, unc6 ? unc6 + 2 : nullptr);
-    face_cons_flux<NVP, 1>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU, unc6 ? unc6 + 3 : nullptr);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU, unc6 ? unc6 + 2 : nullptr);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU, unc6 ? unc6 + 3 : nullptr);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double dp = Wn[v] - Wc[v];
       t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
       dzm[v] = dp;
     }
-    face_cons_flux<NVP, 2>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, unc6 ? unc6 + 4 : nullptr);
-    face_cons_flux<NVP, 2>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, unc6 ? unc6 + 5 : nullptr);
+    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, unc6 ? unc6 + 4 : nullptr);
+    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, unc6 ? unc6 + 5 : nullptr);
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
@@ -768,7 +823,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         const double* const ua[3] = {Uf[1], Uf[3], Uf[4]};
         double* const qo[3] = {qa, qb, qzm};
         double* const io[3] = {&ir6[1], &ir6[3], &ir6[4]};
-        pred_states<5, 3>(P, ua, dU, qo, io);
+        pred_states<5, 3, EOS>(P, ua, dU, qo, io);
 #pragma unroll
         for (int v = 0; v < 7; ++v) {
           X[v * XSTR + xs_own] = qa[v];
@@ -779,7 +834,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         const double* const ub[3] = {Uf[0], Uf[2], Uf[5]};
         double* const qo[3] = {qxm, qym, zpn};
         double* const io[3] = {&ir6[0], &ir6[2], &ir6[5]};
-        pred_states<5, 3>(P, ub, dU, qo, io);
+        pred_states<5, 3, EOS>(P, ub, dU, qo, io);
       }
       double Un[NV];           // U^n of cell p
       {
@@ -788,7 +843,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         Un[1] = rho * Wc[1];
         Un[2] = rho * Wc[2];
         Un[3] = rho * Wc[3];
-        Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), Wc[4] * P.igm1);
+        Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), EOS == HX_EOS_IDEAL ? Wc[4] * P.igm1 : gr_energy(P, rho, Wc[4]));
       }
       if constexpr (NV > 5) {
         // Passive scalars one at a time (R7: mass fractions are reconstructed, rho f is advanced): limited slopes,
@@ -929,19 +984,19 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       predictor(std::integral_constant<int, NV>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, nullptr);
       double q[NF];
       if (wid == TY) {
-        pred_state<NV>(P, Uf[3], dU, q);
+        pred_state<NV, EOS>(P, Uf[3], dU, q);
 #pragma unroll
         for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
       } else if (wid == TY + 1) {
-        pred_state<NV>(P, Uf[2], dU, q);
+        pred_state<NV, EOS>(P, Uf[2], dU, q);
       } else if (wid == TY + 2) {
-        pred_state<NV>(P, Uf[1], dU, q);
+        pred_state<NV, EOS>(P, Uf[1], dU, q);
         if (act) {
 #pragma unroll
           for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
         }
       } else {
-        pred_state<NV>(P, Uf[0], dU, q);
+        pred_state<NV, EOS>(P, Uf[0], dU, q);
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (1)
       if (wid == TY + 1) {
