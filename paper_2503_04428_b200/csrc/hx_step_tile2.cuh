@@ -1,27 +1,32 @@
-// hx_step_tile2.cuh -- the fused 3-D step kernel, second design (A1-A7 of SURVEY 8(a) in ONE pass over HBM).
+// hx_step_tile2.cuh -- the fused 3-D step kernel (A1-A7 of SURVEY 8(a) in ONE pass over HBM), second design.
 //
-// Why a second design: ncu on the first tiled kernel (profiles/r1a_*) showed the FP64 pipe only half
-// busy with the issue port just as loaded (fp64 : other instructions = 1 : 1), 22 % of the threads
-// doing full work on ring cells, and 3 warps per scheduler.  This kernel
-//   * owns a 32 x TY tile per CTA (warp <-> row, lane <-> cell) and marches along z; the one-cell ring
-//     around the tile is handled by THREE extra warps (bottom row, top row, left+right columns) that
-//     run only the part of the scheme the tile needs from them (slopes, predictor, one predicted face
-//     state, at most one Riemann solve);
-//   * exchanges every neighbour quantity through shared memory: limited-slope neighbours are read from
-//     the staged primitive plane, the predicted "+" face state of a cell is written to the cell's own
-//     exchange slot, the neighbour on the other side of that face reads it, solves the Riemann problem
-//     once and writes the flux back INTO THE SAME SLOT, where the first cell picks it up as the flux
-//     through its upper face;
-//   * stages planes (tile + 2 ghost layers, all fields) with one TMA bulk-tensor copy each into a
-//     3-deep ring, so a plane has a whole iteration to arrive;
-//   * trims the arithmetic: reciprocal / square root = MUFU seed + one cubic correction, limiters on
-//     pre-scaled one-sided differences, flux differences accumulated straight into the half-step
-//     increment, tangential momentum and scalar fluxes as (value x mass flux);
-//   * keeps geometry out of registers on bitwise-uniform Cartesian grids (UNI: kernel-parameter
-//     constants), and as per-thread / per-plane 1-D table products otherwise.
+// Why a second design: ncu on the first tiled kernel (profiles/r1a_*) showed the FP64 pipe only half busy with
+// the issue port just as loaded (fp64 : other instructions = 1 : 1), 22 % of the threads doing full work on ring
+// cells, and 3 warps per scheduler.  This kernel
+//   * owns a 32 x 8 tile per CTA (warp <-> row, lane <-> cell) and marches along z; the one-cell ring around the
+//     tile is handled by FOUR extra warps (bottom row, top row, left column, right column) that run only what the
+//     tile needs from them (slopes, half-step increment, one predicted face state, at most one Riemann solve);
+//   * rebalances the register file with setmaxnreg: the ring warpgroup gives registers back, the two owner
+//     warpgroups take them, because ptxas interleaves the owners' independent fp64 chains only with ~190 registers;
+//   * exchanges every neighbour quantity through shared memory: slope neighbours are read from the staged
+//     primitive plane; the predicted "+" face state of a cell goes into the cell's own exchange slot, the
+//     neighbour across that face reads it, solves the Riemann problem once and writes the flux back INTO THE
+//     SAME SLOT, where the first cell picks it up as the flux through its upper face;
+//   * stages planes (tile + 2 ghost layers, all fields) with one TMA bulk-tensor copy each into a 3-deep ring,
+//     and the z-axis tables of the chunk once;
+//   * keeps the owner iteration straight-line (no edge-iteration branches), batches the predicted states and the
+//     three HLLC solves stage by stage, defers the CFL rate of a cell by one plane, and advances passive scalars
+//     one at a time after the hydro fields (register peak);
+//   * trims the arithmetic: reciprocal / square root = MUFU seed + one cubic correction, limiters on pre-scaled
+//     one-sided differences, flux differences accumulated straight into the half-step increment, tangential
+//     momentum and scalar fluxes as (value x mass flux);
+//   * keeps geometry out of registers on bitwise-uniform Cartesian grids (UNI: kernel-parameter constants), and
+//     as per-thread / per-plane 1-D table products otherwise;
+//   * is instantiated for the ideal gas (Eq. 5) and, for nvar 9, for the gas + radiation EOS (Eq. 6-7, Newton-
+//     Raphson for T inside the kernel).
 //
 // PAPER.md: Eq. 17 (slopes), Eq. 18 + Toro 16.5 (unsplit predictor), Eq. 19 (update), L201 (HLL/HLLC),
-// Eq. 13-16 (spherical sources), Eq. 2-3 (gravity); readings R1-R25.
+// Eq. 13-16 (spherical sources), Eq. 2-3 (gravity), Eq. 5-7 (EOS); readings R1-R27.
 #pragma once
 #include <cuda.h>
 
