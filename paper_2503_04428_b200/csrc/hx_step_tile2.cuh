@@ -197,9 +197,11 @@ __device__ __forceinline__ void tma_load_plane(const CUtensorMap* tmap, void* ds
 // a1 T + a4 T^4 = b, by Newton-Raphson as the paper prescribes (L102), from the smaller single-term root (the
 // iterate then only moves down), until the correction is a few ulp (R27); reciprocals by seed + cubic correction.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double gr_temperature(double a1, double a4, double b) {
+// Tg > 0: start from this guess instead (the temperature of the cell centre for its face and predicted states: a
+// start below the root overshoots once and then descends like any other; 2-3 steps instead of 6-8, same root).
+__device__ __forceinline__ double gr_temperature(double a1, double a4, double b, double Tg = 0.0) {
   if (!(b > 0.0)) return b * rcp3(a1);                    // non-physical: T <= 0, hence P <= 0, which the rate check reports
-  double T = dmin(b * rcp3(a1), sqrt3(sqrt3(b * rcp3(a4))));
+  double T = (Tg > 0.0) ? Tg : dmin(b * rcp3(a1), sqrt3(sqrt3(b * rcp3(a4))));
   for (int it = 0; it < 60; ++it) {
     const double T3 = T * T * T;
     const double step = (fma(a4 * T3, T, a1 * T) - b) * rcp3(fma(4.0 * a4, T3, a1));
@@ -209,16 +211,17 @@ __device__ __forceinline__ double gr_temperature(double a1, double a4, double b)
   return T;
 }
 // P and c_s from (rho, 1/rho, e); e from (rho, P)
-__device__ __forceinline__ void gr_from_energy(const Phys& P, double rho, double ir, double e, double& p, double& c) {
-  const double T = gr_temperature(rho * P.rgas * P.igm1, P.arad, e);
+__device__ __forceinline__ void gr_from_energy(const Phys& P, double rho, double ir, double e, double& p, double& c, double Tg = 0.0) {
+  const double T = gr_temperature(rho * P.rgas * P.igm1, P.arad, e, Tg);
   const double T3 = T * T * T;
   const double pg = rho * P.rgas * T;
   p = fma(P.arad * (1.0 / 3.0) * T3, T, pg);
   const double al = P.arad * (1.0 / 3.0) * T3 * ir * rcp3(P.rgas);   // P_r / P_g
   c = sqrt3(fma(al, fma(16.0, al, 20.0), P.gamma * P.igm1) * rcp3(fma(12.0, al, P.igm1)) * P.rgas * T);
 }
-__device__ __forceinline__ double gr_energy(const Phys& P, double rho, double p) {
-  const double T = gr_temperature(rho * P.rgas, P.arad * (1.0 / 3.0), p);
+__device__ __forceinline__ double gr_energy(const Phys& P, double rho, double p, double Tg = 0.0, double* Tout = nullptr) {
+  const double T = gr_temperature(rho * P.rgas, P.arad * (1.0 / 3.0), p, Tg);
+  if (Tout) *Tout = T;
   const double T2 = T * T;
   return fma(P.arad, T2 * T2, rho * P.rgas * T * P.igm1);
 }
@@ -249,7 +252,7 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
 // area/volume coefficient `coef` (Eq. 18: + for the lower face, - for the upper face).
 template <int NV, int DIR, int EOS = HX_EOS_IDEAL>
 __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double sc, double coef, double* Uf, double* dU,
-                                               double* unc_out = nullptr) {
+                                               double* unc_out = nullptr, double Tg = 0.0) {
   double Wf[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) Wf[v] = fma(sc, t[v], Wc[v]);
@@ -259,7 +262,7 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
   Uf[2] = r * Wf[2];
   Uf[3] = r * Wf[3];
   const double ke2 = fma(Uf[3], Wf[3], fma(Uf[2], Wf[2], Uf[1] * Wf[1]));
-  Uf[4] = fma(0.5, ke2, EOS == HX_EOS_IDEAL ? Wf[4] * P.igm1 : gr_energy(P, r, Wf[4]));
+  Uf[4] = fma(0.5, ke2, EOS == HX_EOS_IDEAL ? Wf[4] * P.igm1 : gr_energy(P, r, Wf[4], Tg));
   const double unc = Wf[1 + DIR] * coef;
   if (unc_out) *unc_out = unc;   // signed (dt/2) dS/dV u_n of this face: what a passive scalar's flux rides on
   dU[0] = fma(r, unc, dU[0]);
@@ -278,7 +281,7 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
 // Predicted face state U^{n+1/2} = cons(Wf) + dU (Eq. 18) as the record the Riemann solver consumes:
 // q = rho, u[3], P, E, c_s, scalars f.
 template <int NV, int EOS = HX_EOS_IDEAL>
-__device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, const double* dU, double* q) {
+__device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, const double* dU, double* q, double Tg = 0.0) {
   const double r = Uf[0] + dU[0];
   const double m1 = Uf[1] + dU[1], m2 = Uf[2] + dU[2], m3 = Uf[3] + dU[3];
   const double E = Uf[4] + dU[4];
@@ -294,7 +297,7 @@ __device__ __forceinline__ void pred_state(const Phys& P, const double* Uf, cons
     q[4] = P.gm1 * e;
     q[6] = sqrt3((P.gamma * P.gm1) * ir * e);            // c^2 = gamma P / rho
   } else {
-    gr_from_energy(P, r, ir, e, q[4], q[6]);
+    gr_from_energy(P, r, ir, e, q[4], q[6], Tg);
   }
 #pragma unroll
   for (int s = 5; s < NV; ++s) q[2 + s] = (Uf[s] + dU[s]) * ir;
@@ -395,7 +398,7 @@ __device__ __forceinline__ void sqrt3_n(const double* x, double* y) {
 
 // N predicted face states at once (same arithmetic as pred_state)
 template <int NV, int N, int EOS = HX_EOS_IDEAL>
-__device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q, double* const* ir_out = nullptr) {
+__device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q, double* const* ir_out = nullptr, double Tg = 0.0) {
   double r[N], m1[N], m2[N], m3[N], E[N], mm[N], ir[N], e[N], x[N], c[N];
 #pragma unroll
   for (int k = 0; k < N; ++k) {
@@ -423,7 +426,7 @@ __device__ __forceinline__ void pred_states(const Phys& P, const double* const* 
     for (int k = 0; k < N; ++k) pr[k] = P.gm1 * e[k];
   } else {
 #pragma unroll
-    for (int k = 0; k < N; ++k) gr_from_energy(P, r[k], ir[k], e[k], pr[k], c[k]);
+    for (int k = 0; k < N; ++k) gr_from_energy(P, r[k], ir[k], e[k], pr[k], c[k], Tg);
   }
 #pragma unroll
   for (int k = 0; k < N; ++k) {
@@ -734,7 +737,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   // owners, whose passive scalars follow one at a time to keep the register peak down); unc6: per-face signed
   // (dt/2) dS/dV u_n for that scalar pass.
   auto predictor = [&](auto nvp_tag, const double* Pc, const double* Wn, int pk, double* Wc, double* dU, double* Uxm, double* Uxp,
-                       double* Uym, double* Uyp, double* Uzm, double* Uzp, double& hcm2, double* unc6) {
+                       double* Uym, double* Uyp, double* Uzm, double* Uzp, double& hcm2, double* unc6, double& Tc, double& ec) {
     constexpr int NVP = decltype(nvp_tag)::value;
     double flz, fhz, hcp2;   // per-plane z geometry (uniform addresses)
     if (UNI) {
@@ -752,29 +755,33 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       Wc[v] = Pc[v * FSTR + cidx];
       dU[v] = 0.0;
     }
+    // gas + radiation EOS: temperature and internal energy of the cell centre, the Newton start of its twelve face solves
+    Tc = 0.0;
+    ec = 0.0;
+    if (EOS != HX_EOS_IDEAL) ec = gr_energy(P, Wc[0], Wc[4], 0.0, &Tc);
     double t[NVP];
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
     }
-    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU, unc6 ? unc6 + 0 : nullptr);
-    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU, unc6 ? unc6 + 1 : nullptr);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU, unc6 ? unc6 + 0 : nullptr, Tc);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU, unc6 ? unc6 + 1 : nullptr, Tc);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
     }
-    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU, unc6 ? unc6 + 2 : nullptr);
-    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU, unc6 ? unc6 + 3 : nullptr);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU, unc6 ? unc6 + 2 : nullptr, Tc);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU, unc6 ? unc6 + 3 : nullptr, Tc);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double dp = Wn[v] - Wc[v];
       t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
       dzm[v] = dp;
     }
-    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, unc6 ? unc6 + 4 : nullptr);
-    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, unc6 ? unc6 + 5 : nullptr);
+    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, unc6 ? unc6 + 4 : nullptr, Tc);
+    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, unc6 ? unc6 + 5 : nullptr, Tc);
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
@@ -813,7 +820,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 
     // Edge iterations (p = k0-1 and p = k1) run the same code on valid but unused data; only the global
     // store and the CFL rate are predicated, so the iteration is three straight-line blocks.
-    double Wn[NV], Wc[NV], dU[NV], hcm2;
+    double Wn[NV], Wc[NV], dU[NV], hcm2, Tc, ec;
     double Uf[6][NV];          // conserved face states: 0 x-, 1 x+, 2 y-, 3 y+, 4 z-, 5 z+
     if constexpr (OWN) {
       // ======== block 1: slopes, half-step increment, the six predicted states in two interleaved
@@ -821,14 +828,14 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       cfl_rate(pk - 2);
       convert(Pn, cidx, Wn, true);                       // [A] cons -> prim of the own cell of plane p+1, in place
       double unc[6], ir6[6];   // per face: signed (dt/2) dS/dV u_n of the face state, 1/rho of the predicted state
-      predictor(std::integral_constant<int, 5>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, unc);
+      predictor(std::integral_constant<int, 5>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, unc, Tc, ec);
       double qxm[NF], qym[NF], qzm[NF], zpn[NF];
       {
         double qa[NF], qb[NF];
         const double* const ua[3] = {Uf[1], Uf[3], Uf[4]};
         double* const qo[3] = {qa, qb, qzm};
         double* const io[3] = {&ir6[1], &ir6[3], &ir6[4]};
-        pred_states<5, 3, EOS>(P, ua, dU, qo, io);
+        pred_states<5, 3, EOS>(P, ua, dU, qo, io, Tc);
 #pragma unroll
         for (int v = 0; v < 7; ++v) {
           X[v * XSTR + xs_own] = qa[v];
@@ -839,7 +846,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         const double* const ub[3] = {Uf[0], Uf[2], Uf[5]};
         double* const qo[3] = {qxm, qym, zpn};
         double* const io[3] = {&ir6[0], &ir6[2], &ir6[5]};
-        pred_states<5, 3, EOS>(P, ub, dU, qo, io);
+        pred_states<5, 3, EOS>(P, ub, dU, qo, io, Tc);
       }
       double Un[NV];           // U^n of cell p
       {
@@ -848,7 +855,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         Un[1] = rho * Wc[1];
         Un[2] = rho * Wc[2];
         Un[3] = rho * Wc[3];
-        Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), EOS == HX_EOS_IDEAL ? Wc[4] * P.igm1 : gr_energy(P, rho, Wc[4]));
+        Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), EOS == HX_EOS_IDEAL ? Wc[4] * P.igm1 : ec);
       }
       if constexpr (NV > 5) {
         // Passive scalars one at a time (R7: mass fractions are reconstructed, rho f is advanced): limited slopes,
@@ -986,22 +993,22 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     } else {
       // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
       convert_plane(Pn, Wn);
-      predictor(std::integral_constant<int, NV>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, nullptr);
+      predictor(std::integral_constant<int, NV>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, nullptr, Tc, ec);
       double q[NF];
       if (wid == TY) {
-        pred_state<NV, EOS>(P, Uf[3], dU, q);
+        pred_state<NV, EOS>(P, Uf[3], dU, q, Tc);
 #pragma unroll
         for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
       } else if (wid == TY + 1) {
-        pred_state<NV, EOS>(P, Uf[2], dU, q);
+        pred_state<NV, EOS>(P, Uf[2], dU, q, Tc);
       } else if (wid == TY + 2) {
-        pred_state<NV, EOS>(P, Uf[1], dU, q);
+        pred_state<NV, EOS>(P, Uf[1], dU, q, Tc);
         if (act) {
 #pragma unroll
           for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
         }
       } else {
-        pred_state<NV, EOS>(P, Uf[0], dU, q);
+        pred_state<NV, EOS>(P, Uf[0], dU, q, Tc);
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (1)
       if (wid == TY + 1) {
