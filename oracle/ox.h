@@ -27,7 +27,8 @@ enum { OX_BC_PERIODIC = 0, OX_BC_TRANSMISSIVE = 1, OX_BC_REFLECTING = 2, OX_BC_W
 enum { OX_EOS_IDEAL = 0 /* Eq. 5 */, OX_EOS_GAS_RADIATION = 1 /* Eq. 6-7: ideal gas in equilibrium with radiation */ };
 enum { OX_RIEMANN_HLL = 0, OX_RIEMANN_HLLC = 1 };
 enum { OX_LIM_NONE = 0, OX_LIM_MINMOD = 1, OX_LIM_VANLEER = 2, OX_LIM_VANALBADA = 3, OX_LIM_MC = 4 };
-enum { OX_GRAV_NONE = 0, OX_GRAV_UNIFORM = 1, OX_GRAV_POINT_MASS = 2 };
+enum { OX_GRAV_NONE = 0, OX_GRAV_UNIFORM = 1, OX_GRAV_POINT_MASS = 2,
+       OX_GRAV_SELF = 3 /* Eq. 4: central mass + spherically averaged mass of the grid inside r */ };
 enum { OX_SPACING_UNIFORM = 0, OX_SPACING_LOG = 1, OX_SPACING_CUSTOM = 2 };
 enum { OX_CONSERVED = 0, OX_PRIMITIVE = 1 };
 
@@ -48,6 +49,7 @@ typedef struct {
   double GM;           /* OX_GRAV_POINT_MASS: g = -GM/r_c^2 e_r (spherical only), Eq. 3         */
   double eos_R;        /* OX_EOS_GAS_RADIATION: k_b / mu (gas constant per unit mass), Eq. 6a     */
   double eos_ar;       /* OX_EOS_GAS_RADIATION: radiation constant a_r, Eq. 6a-6b                 */
+  double G;            /* OX_GRAV_SELF: gravitational constant; GM is then G times the central mass M_c */
 } ox_config;
 
 int ox_create(const ox_config* cfg, ox_handle** out);
@@ -71,6 +73,8 @@ int ox_riemann_flux(int riemann, double gamma, int ndim, int ns, int dir, const 
 int ox_physical_flux(double gamma, int ndim, int ns, int dir, const double* U, double* F);
 /* EOS closures for the pins: P(rho, e) (Eq. 5 / Eq. 6 through the Newton-Raphson solve for T, L102), e(rho, P),
  * c_s(rho, P) (Eq. 5 / Eq. 7).  eos = OX_EOS_*; R = k_b/mu and ar are ignored by the ideal gas. */
+/* OX_GRAV_SELF: acceleration g_r(r_c) of interior radial cell i for the CURRENT state (for the pins). */
+int ox_self_gravity(ox_handle* h, int i, double* g_out);
 double ox_eos_pressure(int eos, double gamma, double R, double ar, double rho, double e);
 double ox_eos_energy(int eos, double gamma, double R, double ar, double rho, double P);
 double ox_eos_sound_speed(int eos, double gamma, double R, double ar, double rho, double P);

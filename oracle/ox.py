@@ -14,7 +14,7 @@ CARTESIAN, SPHERICAL = 0, 1
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTING, BC_WEDGE = 0, 1, 2, 3
 RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 LIM_NONE, LIM_MINMOD, LIM_VANLEER, LIM_VANALBADA, LIM_MC = 0, 1, 2, 3, 4
-GRAV_NONE, GRAV_UNIFORM, GRAV_POINT_MASS = 0, 1, 2
+GRAV_NONE, GRAV_UNIFORM, GRAV_POINT_MASS, GRAV_SELF = 0, 1, 2, 3
 SPACING_UNIFORM, SPACING_LOG, SPACING_CUSTOM = 0, 1, 2
 CONSERVED, PRIMITIVE = 0, 1
 OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_NONPHYSICAL, ERR_UNSUPPORTED = 0, -1, -2, -4, -5
@@ -29,7 +29,7 @@ class OxConfig(C.Structure):
         ("eos", C.c_int), ("gamma", C.c_double),
         ("riemann", C.c_int), ("limiter", C.c_int), ("n_scalars", C.c_int),
         ("gravity", C.c_int), ("g", C.c_double * 3), ("GM", C.c_double),
-        ("eos_R", C.c_double), ("eos_ar", C.c_double),
+        ("eos_R", C.c_double), ("eos_ar", C.c_double), ("G", C.c_double),
     ]
 
 
@@ -50,6 +50,7 @@ def lib():
         L.ox_compute_dt.argtypes = [vp, C.c_double, dp]
         L.ox_step.argtypes = [vp, C.c_double]
         L.ox_cell_update.argtypes = [vp, ip, ip, ip, C.c_double, dp]
+        L.ox_self_gravity.argtypes = [vp, ip, C.POINTER(C.c_double)]
         L.ox_riemann_flux.argtypes = [ip, C.c_double, ip, ip, ip, dp, dp, dp]
         for f in (L.ox_eos_pressure, L.ox_eos_energy, L.ox_eos_sound_speed):
             f.argtypes = [ip] + [C.c_double] * 5
@@ -100,6 +101,7 @@ def make_config(spec: dict) -> tuple:
     cfg.eos = int(spec.get("eos", 0))
     cfg.eos_R = float(spec.get("eos_R", 0.0))
     cfg.eos_ar = float(spec.get("eos_ar", 0.0))
+    cfg.G = float(spec.get("G", 0.0))
     cfg.riemann = int(spec.get("riemann", RIEMANN_HLLC))
     cfg.limiter = int(spec.get("limiter", LIM_MINMOD))
     cfg.n_scalars = int(spec.get("n_scalars", 0))
@@ -175,6 +177,13 @@ class Oracle:
         if rc != OK:
             raise OracleError(rc, "ox_cell_update")
         return out
+
+    def self_gravity(self, i: int) -> float:
+        g = C.c_double()
+        rc = self._L.ox_self_gravity(self._h, i, C.byref(g))
+        if rc != OK:
+            raise OracleError(rc, "ox_self_gravity")
+        return g.value
 
     def cell_geometry(self, i, j, k):
         dV = C.c_double()

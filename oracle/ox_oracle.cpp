@@ -50,6 +50,9 @@ struct ox_handle {
   size_t ncp;              // padded cells
   std::vector<double> xf[3];  // padded face coordinates, xf[d][idx + ng[d]] = minus face of cell idx
   std::vector<double> U;      // conserved state, [nvar][np2][np1][np0]
+  std::vector<double> gself;  // OX_GRAV_SELF: g_r at the centres of the interior radial cells, for the state in U
+  double gself_mtot = 0.0;    // ... and G times the whole enclosed mass (cells beyond the outer radius)
+  bool gself_dirty = true;
 
   size_t cell(int i, int j, int k) const {
     return ((size_t)(k + ng[2]) * np[1] + (size_t)(j + ng[1])) * np[0] + (size_t)(i + ng[0]);
@@ -105,7 +108,45 @@ double gravity_raw(const ox_handle* h, int d, int idx) {
     const double rc = h->xc(0, idx);
     return -h->c.GM / (rc * rc);
   }
+  if (h->c.gravity == OX_GRAV_SELF) {   // Eq. 4 with the table refresh_self_gravity() made for the current state
+    if (d != 0) return 0.0;
+    if (idx >= 0 && idx < h->c.n[0]) return h->gself[idx];
+    const double rc = h->xc(0, idx);
+    return -(idx < 0 ? h->c.GM : h->gself_mtot) / (rc * rc);   // inside r_min: the central mass only; outside r_max: everything
+  }
   return 0.0;
+}
+
+// Eq. 4 (L73-L77): g(r, t) = -G M(r, t) / r^2 e_r, "M(r,t) the total mass within the sphere of radius r", "in the
+// approximation of a spherically symmetric matter distribution".  Reading R28: at the centre r_c of radial cell i
+//   M = M_c + (4 pi / dOmega) [ sum_{i' < i} m_i' + m_i (r_c^3 - r_-^3) / (r_+^3 - r_-^3) ],   m_i = sum_{j,k} rho dV,
+// dOmega the solid angle of the grid (the wedge stands for the whole sphere), the shell of cell i counted up to r_c
+// by volume; the field of the state at the START of a step is used for the whole step.
+void refresh_self_gravity(ox_handle* h) {
+  if (h->c.gravity != OX_GRAV_SELF || !h->gself_dirty) return;
+  const ox_config& c = h->c;
+  const int n0 = c.n[0];
+  std::vector<double> m(n0, 0.0);
+  for (int k = 0; k < c.n[2]; ++k)
+    for (int j = 0; j < c.n[1]; ++j)
+      for (int i = 0; i < n0; ++i) {
+        double dV, dS[3][2];
+        cell_geometry(h, i, j, k, dV, dS);
+        m[i] += h->U[h->cell(i, j, k)] * dV;
+      }
+  const double PI = 3.14159265358979323846;
+  const double domega = (std::cos(h->fm(1, 0)) - std::cos(h->fp(1, c.n[1] - 1))) * (h->fp(2, c.n[2] - 1) - h->fm(2, 0));
+  const double scale = c.G * 4.0 * PI / domega;
+  h->gself.assign(n0, 0.0);
+  double below = 0.0;
+  for (int i = 0; i < n0; ++i) {
+    const double rm = h->fm(0, i), rp = h->fp(0, i), rc = h->xc(0, i);
+    const double frac = (rc * rc * rc - rm * rm * rm) / (rp * rp * rp - rm * rm * rm);
+    h->gself[i] = -(c.GM + scale * (below + m[i] * frac)) / (rc * rc);
+    below += m[i];
+  }
+  h->gself_mtot = c.GM + scale * below;
+  h->gself_dirty = false;
 }
 double gravity(const ox_handle* h, int d, int idx) {
   if (h->c.gravity == OX_GRAV_NONE || d >= h->c.ndim) return 0.0;
@@ -526,8 +567,8 @@ int check_config(const ox_config* c) {
   if (c->riemann != OX_RIEMANN_HLL && c->riemann != OX_RIEMANN_HLLC) return OX_ERR_INVALID_ARG;
   if (c->limiter < OX_LIM_NONE || c->limiter > OX_LIM_MC) return OX_ERR_INVALID_ARG;
   if (c->n_scalars < 0 || 2 + c->ndim + c->n_scalars > NVMAX) return OX_ERR_INVALID_ARG;
-  if (c->gravity < OX_GRAV_NONE || c->gravity > OX_GRAV_POINT_MASS) return OX_ERR_INVALID_ARG;
-  if (c->gravity == OX_GRAV_POINT_MASS && c->coords != OX_SPHERICAL) return OX_ERR_INVALID_ARG;
+  if (c->gravity < OX_GRAV_NONE || c->gravity > OX_GRAV_SELF) return OX_ERR_INVALID_ARG;
+  if ((c->gravity == OX_GRAV_POINT_MASS || c->gravity == OX_GRAV_SELF) && c->coords != OX_SPHERICAL) return OX_ERR_INVALID_ARG;
   for (int d = 0; d < 3; ++d) {
     if (d < c->ndim) {
       if (c->n[d] < NG) return OX_ERR_INVALID_ARG;
@@ -631,6 +672,7 @@ int ox_num_threads(void) {
 
 int ox_set_state(ox_handle* h, const double* data, int form) {
   if (!h || !data || (form != OX_CONSERVED && form != OX_PRIMITIVE)) return OX_ERR_INVALID_ARG;
+  h->gself_dirty = true;
   const ox_config& c = h->c;
   const size_t nint = (size_t)c.n[0] * c.n[1] * c.n[2];
 #pragma omp parallel for if (h->ncp > 32768)
@@ -719,6 +761,7 @@ int ox_step(ox_handle* h, double dt) {
   const size_t ncp = h->ncp;
   std::vector<double>& U = h->U;
 
+  refresh_self_gravity(h);   // Eq. 4 from U^n (reading R28)
   fill_ghosts(h, U);  // O0
 
   std::vector<double> W((size_t)nvar * ncp);  // O1 on every padded cell
@@ -816,6 +859,7 @@ int ox_step(ox_handle* h, double dt) {
         for (int v = 0; v < nvar; ++v) Unew[(size_t)v * ncp + ci] = out[v];
       }
   U.swap(Unew);
+  h->gself_dirty = true;
   return OX_OK;
 }
 
@@ -823,6 +867,7 @@ int ox_cell_update(ox_handle* h, int i, int j, int k, double dt, double* out) {
   if (!h || !out || !(dt > 0.0)) return OX_ERR_INVALID_ARG;
   const ox_config& c = h->c;
   if (i < 0 || i >= c.n[0] || j < 0 || j >= c.n[1] || k < 0 || k >= c.n[2]) return OX_ERR_INVALID_ARG;
+  refresh_self_gravity(h);
   double Un[NVMAX], Fm[3][NVMAX], Fp[3][NVMAX];
   naive_get_U(h, i, j, k, Un);
   for (int d = 0; d < c.ndim; ++d) {
@@ -854,6 +899,13 @@ int ox_physical_flux(double gamma, int ndim, int ns, int dir, const double* U, d
   return OX_OK;
 }
 
+
+int ox_self_gravity(ox_handle* h, int i, double* g_out) {
+  if (!h || !g_out || h->c.gravity != OX_GRAV_SELF || i < 0 || i >= h->c.n[0]) return OX_ERR_INVALID_ARG;
+  refresh_self_gravity(h);
+  *g_out = h->gself[i];
+  return OX_OK;
+}
 
 double ox_eos_pressure(int eos, double gamma, double R, double ar, double rho, double e) { return eos_pressure(Eos(eos, gamma, R, ar), rho, e); }
 double ox_eos_energy(int eos, double gamma, double R, double ar, double rho, double P) { return eos_energy(Eos(eos, gamma, R, ar), rho, P); }

@@ -549,6 +549,9 @@ CASES_P11 = [
     ("c3d_rad", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 2),
     ("s3d_rad", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 2),
     ("c1d_hll_rad", 1, [9], 0, [1], [2], 0, 2, 0, 0),
+    # self-gravity (Eq. 4; gravity code 3): central mass + spherically averaged mass of the grid
+    ("s3d_selfgrav", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 3, 1, 1, 1),
+    ("s1d_selfgrav", 1, [8], 1, [2], [1], 3, 4, 1, 0),
 ]
 
 
@@ -570,6 +573,8 @@ def random_problem(ox, case, seed=0):
         kw.update(gravity=ox.GRAV_UNIFORM, g=[0.3, -0.2, -0.5])
     elif grav == 2:
         kw.update(gravity=ox.GRAV_POINT_MASS, GM=0.8)
+    elif grav == 3:
+        kw.update(gravity=ox.GRAV_SELF, GM=0.8, G=0.6)
     if name.endswith("_rad"):
         kw.update(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0)
     spec = wl._spec(name, ndim, n, faces, bc_lo, bc_hi, 1.4, lim, **kw)
@@ -880,3 +885,66 @@ def test_p12_gas_radiation_conserves_and_keeps_uniform_states(oxlib):
     Ua = o.get_state()
     run_steps(o, 0.4, 5)
     assert np.max(np.abs(o.get_state() - Ua)) <= 1e-14 * np.max(np.abs(Ua))
+
+
+# ------------------------------------------------------------------------------------------ P13: self-gravity
+def _shell_problem(ox, n, theta, phi, rho, G=2.0, GM=0.7):
+    fr = wl.log_faces(0.5, 3.0, n[0])
+    faces = [fr, wl.uniform_faces(*theta, n[1]), wl.uniform_faces(*phi, n[2])]
+    spec = wl._spec("selfgrav", 3, list(n), faces, [2, 3, 3], [1, 3, 3], 1.4, wl.LIM_MINMOD, coords=wl.SPHERICAL,
+                    gravity=wl.GRAV_SELF, GM=GM, G=G)
+    rc = 0.5 * (fr[1:] + fr[:-1])
+    W = np.zeros((5, n[2], n[1], n[0]))
+    W[0] = rho(rc)[None, None, :]
+    W[4] = 1.0
+    return spec, W, rc
+
+
+def test_p13_self_gravity_of_a_uniform_shell_is_the_closed_form(oxlib):
+    """Eq. 4 (L73-L77): for uniform density rho between r_min and r, M(r) = M_c + (4 pi / 3) rho (r^3 - r_min^3)
+    whatever the solid angle of the wedge (reading R28: the wedge stands for the whole sphere; the shell of the cell
+    is counted up to its centre by volume)."""
+    ox = oxlib
+    for theta, phi in (((1.0, 1.9), (-0.3, 0.5)), ((0.4, 2.6), (0.0, 3.0))):
+        spec, W, rc = _shell_problem(ox, (40, 6, 5), theta, phi, lambda r: 1.3 + 0.0 * r)
+        o = make(ox, spec, W)
+        exact = -(0.7 + 2.0 * 4.0 / 3.0 * math.pi * 1.3 * (rc ** 3 - 0.5 ** 3)) / rc ** 2
+        got = np.array([o.self_gravity(i) for i in range(40)])
+        assert np.max(np.abs(got / exact - 1.0)) <= 1e-14
+
+
+def test_p13_self_gravity_power_law_and_limits(oxlib):
+    """rho = r^-2: M(r) - M_c = 4 pi (r - r_min) exactly; the cell sums converge to it at second order.  G = 0 is the
+    point mass of Eq. 3, step for step."""
+    ox = oxlib
+    errs = []
+    for n in (40, 80):
+        spec, W, rc = _shell_problem(ox, (n, 4, 4), (1.0, 1.9), (-0.3, 0.5), lambda r: r ** -2.0)
+        o = make(ox, spec, W)
+        exact = -(0.7 + 2.0 * 4.0 * math.pi * (rc - 0.5)) / rc ** 2
+        errs.append(max(abs(o.self_gravity(i) / exact[i] - 1.0) for i in range(n)))
+    assert errs[0] < 1e-2 and errs[1] < errs[0] / 3.0, errs
+    case = ("s3d", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 2)
+    spec, W = random_problem(ox, case)
+    a = make(ox, spec, W)
+    b = make(ox, dict(spec, gravity=wl.GRAV_SELF, G=0.0), W)
+    for _ in range(3):
+        dt = a.compute_dt(0.4)
+        a.step(dt)
+        b.step(dt)
+    assert np.array_equal(a.get_state(), b.get_state())
+
+
+def test_p13_self_gravity_accelerates_a_static_shell_by_rho_g_dt(oxlib):
+    """Uniform pressure, gas at rest: after one small step the radial momentum is dt rho g(r) (sign, use in predictor
+    and update) and nothing else has moved."""
+    ox = oxlib
+    spec, W, rc = _shell_problem(ox, (32, 4, 4), (1.0, 1.9), (-0.3, 0.5), lambda r: 1.0 + 0.2 * np.sin(r))
+    o = make(ox, spec, W)
+    g = np.array([o.self_gravity(i) for i in range(32)])
+    dt = 1e-4 * o.compute_dt(0.5)
+    o.step(dt)
+    U = o.get_state()
+    expect = dt * W[0, 0, 0, :] * g
+    assert np.max(np.abs(U[1, 1, 1, 1:-1] / expect[1:-1] - 1.0)) <= 1e-3
+    assert np.max(np.abs(U[2])) <= 1e-12 and np.max(np.abs(U[3])) <= 1e-12
