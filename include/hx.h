@@ -36,7 +36,8 @@ enum { HX_EOS_IDEAL = 0 /* Eq. 5 */, HX_EOS_GAS_RADIATION = 1 /* Eq. 6-7: ideal 
 enum { HX_RIEMANN_HLL = 0, HX_RIEMANN_HLLC = 1 };       /* L201 */
 /* Slope limiters (L189) + first order (HX_LIM_NONE) + monotonised central (BASELINE.json configs) */
 enum { HX_LIM_NONE = 0, HX_LIM_MINMOD = 1, HX_LIM_VANLEER = 2, HX_LIM_VANALBADA = 3, HX_LIM_MC = 4 };
-enum { HX_GRAV_NONE = 0, HX_GRAV_UNIFORM = 1 /* Eq. 2 */, HX_GRAV_POINT_MASS = 2 /* Eq. 3 */ };
+enum { HX_GRAV_NONE = 0, HX_GRAV_UNIFORM = 1 /* Eq. 2 */, HX_GRAV_POINT_MASS = 2 /* Eq. 3 */,
+       HX_GRAV_SELF = 3 /* Eq. 4: central mass + spherically averaged mass of the grid inside r, refreshed every step */ };
 enum { HX_SPACING_UNIFORM = 0, HX_SPACING_LOG = 1, HX_SPACING_CUSTOM = 2 };   /* L149 */
 enum { HX_HOST = 0, HX_DEVICE = 1 };
 enum { HX_CONSERVED = 0, HX_PRIMITIVE = 1 };
@@ -60,11 +61,12 @@ typedef struct {
   int eos;                /* HX_EOS_IDEAL or HX_EOS_GAS_RADIATION (T from e by Newton-Raphson, L102)         */
   double gamma;           /* adiabatic index > 1                                                     */
   int riemann, limiter, n_scalars;
-  int gravity;            /* HX_GRAV_*; point mass needs HX_SPHERICAL                                */
+  int gravity;            /* HX_GRAV_*; point mass and self-gravity need HX_SPHERICAL                */
   double g[3];            /* uniform: acceleration vector (force = +rho*g, R12)            */
   double GM;              /* point mass: g = -GM/r_c^2 e_r                                           */
   double eos_R;           /* HX_EOS_GAS_RADIATION: k_b / mu, gas constant per unit mass (Eq. 6a); > 0         */
   double eos_ar;          /* HX_EOS_GAS_RADIATION: radiation constant a_r (Eq. 6a-6b); > 0                    */
+  double G;               /* HX_GRAV_SELF: gravitational constant (GM is then G times the central mass)      */
 } hx_config;
 
 /* Validate cfg, allocate the padded double-buffered state and the geometry tables on the current

@@ -94,6 +94,99 @@ cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, cons
   return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------
+// Self-gravity (Eq. 4; R28): g_r(r_c,i) = -[G M_c + G (4 pi / dOmega) (sum_{i'<i} m_i'
+// + m_i (r_c^3 - r_-^3)/(r_+^3 - r_-^3))] / r_c^2 with the shell masses m_i = sum_{j,k} rho dV of the CURRENT state.
+// Stage 1: each block sums rho x (theta weight) x (phi weight) over a fixed set of (j,k) rows for 256 radial
+// cells (coalesced along r); stage 2: one block adds the partial sums in block order (deterministic), scans
+// over r and rewrites the radial acceleration table, ghost entries included (mirror image behind a reflecting
+// face, R25; central mass only inside r_min; everything outside r_max).
+// ---------------------------------------------------------------------------------------------
+struct SelfGrav {
+  const double* xf[3];   // padded face coordinates of the three axes (device)
+  double* partial;       // [nrows_groups][n0]
+  double* grav_r;        // the table T.grav[0], np[0] entries
+  double GM, G;
+  int groups, bc_lo, bc_hi;
+};
+
+__global__ void shell_mass_partial_kernel(Layout L, const double* __restrict__ U, SelfGrav sg) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= L.n[0]) return;
+  const int rows = L.n[1] * L.n[2];
+  double acc = 0.0;
+  for (int r = blockIdx.y; r < rows; r += gridDim.y) {
+    const int j = r % L.n[1], k = r / L.n[1];
+    const double wt = cos(sg.xf[1][j + L.ng[1]]) - cos(sg.xf[1][j + L.ng[1] + 1]);
+    const double wp = sg.xf[2][k + L.ng[2] + 1] - sg.xf[2][k + L.ng[2]];
+    acc = fma(U[L.off(i + L.ng[0], j + L.ng[1], k + L.ng[2])], wt * wp, acc);
+  }
+  sg.partial[(size_t)blockIdx.y * L.n[0] + i] = acc;
+}
+
+__global__ void self_gravity_table_kernel(Layout L, SelfGrav sg) {
+  extern __shared__ double sm[];            // m[n0], then g[n0]
+  double* m = sm;
+  double* g = sm + L.n[0];
+  const int n0 = L.n[0];
+  for (int i = threadIdx.x; i < n0; i += blockDim.x) {
+    double s = 0.0;
+    for (int b = 0; b < sg.groups; ++b) s += sg.partial[(size_t)b * n0 + i];
+    const double rm = sg.xf[0][i + L.ng[0]], rp = sg.xf[0][i + L.ng[0] + 1];
+    m[i] = s * ((rp * rp * rp - rm * rm * rm) / 3.0);
+  }
+  __syncthreads();
+  __shared__ double mtot;
+  if (threadIdx.x == 0) {
+    const double PI = 3.14159265358979323846;
+    const double domega = (cos(sg.xf[1][L.ng[1]]) - cos(sg.xf[1][L.ng[1] + L.n[1]])) * (sg.xf[2][L.ng[2] + L.n[2]] - sg.xf[2][L.ng[2]]);
+    const double scale = sg.G * 4.0 * PI / domega;
+    double below = 0.0;
+    for (int i = 0; i < n0; ++i) {
+      const double rm = sg.xf[0][i + L.ng[0]], rp = sg.xf[0][i + L.ng[0] + 1], rc = 0.5 * (rm + rp);
+      const double frac = (rc * rc * rc - rm * rm * rm) / (rp * rp * rp - rm * rm * rm);
+      g[i] = -(sg.GM + scale * (below + m[i] * frac)) / (rc * rc);
+      below += m[i];
+    }
+    mtot = sg.GM + scale * below;
+  }
+  __syncthreads();
+  for (int p = threadIdx.x; p < L.np[0]; p += blockDim.x) {
+    const int i = p - L.ng[0];
+    const double rc = 0.5 * (sg.xf[0][p] + sg.xf[0][p + 1]);
+    const bool refl_lo = sg.bc_lo == HX_BC_REFLECTING || sg.bc_lo == HX_BC_WEDGE, refl_hi = sg.bc_hi == HX_BC_REFLECTING || sg.bc_hi == HX_BC_WEDGE;
+    double v;
+    if (i < 0) v = refl_lo ? -g[-1 - i] : -sg.GM / (rc * rc);
+    else if (i >= n0) v = refl_hi ? -g[2 * n0 - 1 - i] : -mtot / (rc * rc);
+    else v = g[i];
+    sg.grav_r[p] = v;
+  }
+}
+
+cudaError_t launch_self_gravity(const Layout& L, const double* U, const double* const xf[3], double* partial, int groups, double* grav_r,
+                                double GM, double G, int bc_lo, int bc_hi, cudaStream_t s) {
+  SelfGrav sg;
+  for (int d = 0; d < 3; ++d) sg.xf[d] = xf[d];
+  sg.partial = partial;
+  sg.grav_r = grav_r;
+  sg.GM = GM;
+  sg.G = G;
+  sg.groups = groups;
+  sg.bc_lo = bc_lo;
+  sg.bc_hi = bc_hi;
+  dim3 grid((unsigned)((L.n[0] + 255) / 256), (unsigned)groups);
+  shell_mass_partial_kernel<<<grid, 256, 0, s>>>(L, U, sg);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const size_t smem = 2 * (size_t)L.n[0] * sizeof(double);
+  if (smem > 48 * 1024) {
+    e = cudaFuncSetAttribute(self_gravity_table_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  self_gravity_table_kernel<<<1, 256, smem, s>>>(L, sg);
+  return cudaGetLastError();
+}
+
 // interior SoA [nvar][n2][n1][n0] (caller layout)  ->  padded state; to_cons: input is primitive
 template <int ND>
 __global__ void pack_kernel(Layout L, Phys P, const double* __restrict__ src, double* __restrict__ U, int to_cons) {

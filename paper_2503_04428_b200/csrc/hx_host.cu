@@ -16,6 +16,8 @@ cudaError_t launch_unpack(const Layout& L, const Phys& P, const double* U, doubl
 cudaError_t launch_rate(const Layout& L, const Tables& T, const Phys& P, const double* U, unsigned long long* rate_bits, int* status,
                         cudaStream_t s);
 cudaError_t launch_step_generic(const StepArgs& a, cudaStream_t s);
+cudaError_t launch_self_gravity(const Layout& L, const double* U, const double* const xf[3], double* partial, int groups, double* grav_r,
+                                double GM, double G, int bc_lo, int bc_hi, cudaStream_t s);
 namespace t2 { struct Plan; }
 int tile2_supported(const Layout& L, const Phys& P);
 cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, t2::Plan** out);
@@ -45,6 +47,10 @@ struct hx_handle {
   cudaStream_t stream = nullptr;
   cudaStream_t side = nullptr;    // reads the CFL rate back while the next ghost fill already runs on `stream`
   cudaEvent_t ev_step = nullptr;  // recorded right after the step kernel
+  const double* d_xf[3] = {nullptr, nullptr, nullptr};   // padded face coordinates on the device (self-gravity)
+  double* d_grav_r = nullptr;     // the radial acceleration table inside d_tables (rewritten every step by self-gravity)
+  double* d_sg_partial = nullptr; // self-gravity: partial shell sums [sg_groups][n0]
+  int sg_groups = 0;
   bool ghosts_valid = false;      // ghost layers of d_U[cur] are filled (hx_step fills them eagerly for the next step)
   bool rate_valid = false;
   int kernel_opt = HX_KERNEL_AUTO;
@@ -86,8 +92,9 @@ const char* check_config(const hx_config* c, int* code) {
   if (c->riemann != HX_RIEMANN_HLL && c->riemann != HX_RIEMANN_HLLC) return "unknown Riemann solver";
   if (c->limiter < HX_LIM_NONE || c->limiter > HX_LIM_MC) return "unknown limiter";
   if (c->n_scalars < 0 || 2 + c->ndim + c->n_scalars > NVMAX) return "too many passive scalars";
-  if (c->gravity < HX_GRAV_NONE || c->gravity > HX_GRAV_POINT_MASS) return "unknown gravity type";
-  if (c->gravity == HX_GRAV_POINT_MASS && c->coords != HX_SPHERICAL) return "point-mass gravity needs spherical coordinates";
+  if (c->gravity < HX_GRAV_NONE || c->gravity > HX_GRAV_SELF) return "unknown gravity type";
+  if ((c->gravity == HX_GRAV_POINT_MASS || c->gravity == HX_GRAV_SELF) && c->coords != HX_SPHERICAL)
+    return "point-mass gravity and self-gravity need spherical coordinates";
   for (int d = 0; d < 3; ++d) {
     if (d >= c->ndim) {
       if (c->n[d] != 1) return "inactive directions must have n = 1";
@@ -182,7 +189,7 @@ int build_tables(hx_handle* h) {
   // gravity seen by each cell of each active axis, mirrored behind reflecting faces (R25)
   auto g_raw = [&](int d, int idx_int) -> double {
     if (c.gravity == HX_GRAV_UNIFORM) return c.g[d];
-    if (c.gravity == HX_GRAV_POINT_MASS && d == 0) {
+    if ((c.gravity == HX_GRAV_POINT_MASS || c.gravity == HX_GRAV_SELF) && d == 0) {   // self-gravity: start value, rewritten every step
       const int p = idx_int + L.ng[0];
       const double rc = 0.5 * (xf[0][p] + xf[0][p + 1]);
       return -c.GM / (rc * rc);
@@ -233,6 +240,11 @@ int build_tables(hx_handle* h) {
     for (int p = 0; p < L.np[2]; ++p) pool[idphi + p] = 1.0 / (xf[2][p + 1] - xf[2][p]);
   }
 
+  size_t xfo[3];
+  for (int d = 0; d < 3; ++d) {   // padded face coordinates (self-gravity kernels)
+    xfo[d] = pool.size();
+    pool.insert(pool.end(), xf[d].begin(), xf[d].end());
+  }
   // Bitwise-uniform Cartesian grid (e.g. 2^k cells on a dyadic extent): every cell of an axis has the same
   // hw, 1/width and 1/(centre distance), so the step kernel may take them as constants without changing a bit.
   h->uniform = !sph && c.ndim == 3;
@@ -251,6 +263,8 @@ int build_tables(hx_handle* h) {
   e = cudaMemcpy(h->d_tables, pool.data(), bytes, cudaMemcpyHostToDevice);
   if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpy(tables)");
   const double* base = h->d_tables;
+  for (int d = 0; d < 3; ++d) h->d_xf[d] = base + xfo[d];
+  h->d_grav_r = h->d_tables + grav[0];
   Tables& T = h->T;
   for (int d = 0; d < 3; ++d) {
     for (int s = 0; s < 2; ++s)
@@ -367,6 +381,11 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
       cudaEventCreateWithFlags(&h->ev_step, cudaEventDisableTiming) != cudaSuccess) { hx_destroy(h); return HX_ERR_CUDA; }
   const int rc = build_tables(h);
   if (rc != HX_OK) { hx_destroy(h); return rc; }
+  if (cfg->gravity == HX_GRAV_SELF) {
+    const long long rows = (long long)L.n[1] * L.n[2];
+    h->sg_groups = (int)(rows < 296 ? rows : 296);
+    if (cudaMalloc(&h->d_sg_partial, (size_t)h->sg_groups * L.n[0] * sizeof(double)) != cudaSuccess) { hx_destroy(h); return HX_ERR_ALLOC; }
+  }
   h->cfg.faces[0] = h->cfg.faces[1] = h->cfg.faces[2] = nullptr;   // caller arrays are not retained
   *out = h;
   return HX_OK;
@@ -381,6 +400,7 @@ int hx_destroy(hx_handle* h) {
   if (h->ev1) cudaEventDestroy(h->ev1);
   for (int b = 0; b < 2; ++b)
     if (h->d_U[b]) cudaFree(h->d_U[b]);
+  if (h->d_sg_partial) cudaFree(h->d_sg_partial);
   if (h->d_tables) cudaFree(h->d_tables);
   if (h->d_scal) cudaFree(h->d_scal);
   if (h->h_scal) cudaFreeHost(h->h_scal);
@@ -517,6 +537,12 @@ int hx_step(hx_handle* h, double dt) {
     e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: ghost fill");
     h->launches++;
+  }
+  if (h->cfg.gravity == HX_GRAV_SELF) {   // Eq. 4 from U^n: shell masses, scan over r, new radial acceleration table
+    e = launch_self_gravity(L, h->d_U[h->cur], h->d_xf, h->d_sg_partial, h->sg_groups, h->d_grav_r, h->cfg.GM, h->cfg.G, h->cfg.bc_lo[0],
+                            h->cfg.bc_hi[0], h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: self-gravity");
+    h->launches += 2;
   }
   e = cudaMemsetAsync(&h->d_scal->rate_bits, 0, sizeof(unsigned long long), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: memset");

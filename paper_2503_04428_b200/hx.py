@@ -18,7 +18,7 @@ BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTING, BC_WEDGE = 0, 1, 2, 3
 EOS_IDEAL, EOS_GAS_RADIATION = 0, 1
 RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 LIM_NONE, LIM_MINMOD, LIM_VANLEER, LIM_VANALBADA, LIM_MC = 0, 1, 2, 3, 4
-GRAV_NONE, GRAV_UNIFORM, GRAV_POINT_MASS = 0, 1, 2
+GRAV_NONE, GRAV_UNIFORM, GRAV_POINT_MASS, GRAV_SELF = 0, 1, 2, 3
 SPACING_UNIFORM, SPACING_LOG, SPACING_CUSTOM = 0, 1, 2
 HOST, DEVICE = 0, 1
 CONSERVED, PRIMITIVE = 0, 1
@@ -39,7 +39,7 @@ class HxConfig(C.Structure):
         ("eos", C.c_int), ("gamma", C.c_double),
         ("riemann", C.c_int), ("limiter", C.c_int), ("n_scalars", C.c_int),
         ("gravity", C.c_int), ("g", C.c_double * 3), ("GM", C.c_double),
-        ("eos_R", C.c_double), ("eos_ar", C.c_double),
+        ("eos_R", C.c_double), ("eos_ar", C.c_double), ("G", C.c_double),
     ]
 
 
@@ -111,6 +111,7 @@ def make_config(spec: dict):
     cfg.eos = int(spec.get("eos", EOS_IDEAL))
     cfg.eos_R = float(spec.get("eos_R", 0.0))
     cfg.eos_ar = float(spec.get("eos_ar", 0.0))
+    cfg.G = float(spec.get("G", 0.0))
     cfg.gamma = float(spec["gamma"])
     cfg.riemann = int(spec.get("riemann", RIEMANN_HLLC))
     cfg.limiter = int(spec.get("limiter", LIM_MINMOD))

@@ -229,6 +229,16 @@ def wedge_3d_rad(n=(1024, 256, 256), seed=1005):
     return spec, W
 
 
+def wedge_3d_selfgrav(n=(1024, 256, 256), seed=1005):
+    """the C5 wedge with the self-gravity of its envelope (Eq. 4) on top of the
+    central mass: G M_c = 1 as in wedge_3d, G = 0.004, so that the spherically averaged envelope (mass 8 pi (sqrt(r) - 1)
+    inside r for rho = r^-2.5) adds G M_env ~ 0.9 at r = 100, comparable to the central mass.  Same primitive
+    fields as wedge_3d (its pressure balances the central mass only: the envelope starts to contract slowly)."""
+    spec, W = wedge_3d(n, seed)
+    spec = dict(spec, name="wedge_3d_selfgrav", gravity=GRAV_SELF, G=0.004)
+    return spec, W
+
+
 CONFIGS = {"sod_1d": sod_1d, "kh_2d": kh_2d, "sedov_3d": sedov_3d, "rt_3d": rt_3d, "wedge_3d": wedge_3d}
 
 

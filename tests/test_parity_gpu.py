@@ -58,6 +58,7 @@ REDUCED = {
     "wedge_3d": lambda: wl.wedge_3d((104, 22, 26)),
     "sedov_wedge_3d": lambda: wl.sedov_wedge_3d((72, 40, 36)),   # SURVEY 8(f) rank 3 (Sect. 4.3)
     "wedge_3d_rad": lambda: wl.wedge_3d_rad((72, 18, 20)),        # SURVEY 8(f) rank 1 (gas + radiation EOS, Eq. 6-7)
+    "wedge_3d_selfgrav": lambda: wl.wedge_3d_selfgrav((72, 18, 20)),   # SURVEY 8(f) rank 4 (self-gravity, Eq. 4)
 }
 
 
@@ -259,6 +260,7 @@ FULL = {
     "wedge_3d": (lambda: wl.wedge_3d((1024, 256, 256)), "tile2"),
     "sedov_wedge_3d": (lambda: wl.sedov_wedge_3d(256), "tile2"),
     "wedge_3d_rad": (lambda: wl.wedge_3d_rad((512, 128, 128)), "tile2_rad"),   # gas + radiation EOS: a quarter-size wedge
+    "wedge_3d_selfgrav": (lambda: wl.wedge_3d_selfgrav((512, 128, 128)), "tile2"),   # self-gravity: a quarter-size wedge
 }
 
 
@@ -314,7 +316,7 @@ def test_full_size_sampled_parity(hx, oxlib, name):
         extra = [(n[0] // 2 + a, n[1] // 2 + b, n[2] // 2 + c) for a in range(-5, 5) for b in (-4, -1, 0, 3) for c in (-4, 0, 3)]
     elif name == "rt_3d":       # the perturbed interface slab around z = 1
         extra = [(37 * q % n[0], 91 * q % n[1], n[2] // 2 + c) for q in range(40) for c in (-14, -2, -1, 0, 1, 13)]
-    elif name == "wedge_3d_rad":
+    elif name in ("wedge_3d_rad", "wedge_3d_selfgrav"):
         extra = [(a, 53 * a % n[1], 29 * a % n[2]) for a in list(range(0, 8)) + [81, 82, 154, 155, 236, 237]]
     elif name == "sedov_wedge_3d":   # the blast region around (r0, theta0, phi0) = mid-domain
         extra = [(n[0] // 2 + a, n[1] // 2 + b, n[2] // 2 + c) for a in range(-5, 5) for b in (-4, -1, 0, 3) for c in (-4, 0, 3)]
