@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libhx.so")
 SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_probe.cu",
-           "hx_step_tile2.cu", "hx_step_tile2_nv5.cu", "hx_step_tile2_nv6.cu", "hx_step_tile2_nv7.cu", "hx_step_tile2_nv9.cu"]
+           "hx_step_tile2.cu", "hx_step_tile2_nv5.cu", "hx_step_tile2_nv6.cu", "hx_step_tile2_nv7.cu", "hx_step_tile2_nv9.cu", "hx_step_tile2_nv9_rad.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -3,15 +3,11 @@
 #include "hx_step_tile2_launch.cuh"
 namespace hx {
 namespace t2 {
+cudaError_t launch_nv9_rad(Plan& plan, const Args& a, int cur, cudaStream_t st);
 template <>
 cudaError_t launch_nv<9>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   const Phys& P = a.s.P;
-  if (P.eos == HX_EOS_GAS_RADIATION) {   // Eq. 6-7 (wedge_3d_rad): spherical or Cartesian, limiter and solver at run time
-    if (P.spherical && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
-      return launch_cfg<9, true, GRAV_ANY, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
-    if (P.spherical) return launch_cfg<9, true, GRAV_ANY, -1, -1, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
-    return launch_cfg<9, false, GRAV_ANY, -1, -1, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
-  }
+  if (P.eos == HX_EOS_GAS_RADIATION) return launch_nv9_rad(plan, a, cur, st);   // Eq. 6-7: own translation unit (compile time)
   if (P.spherical && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
     return launch_cfg<9, true, GRAV_ANY, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);
   return launch_generic<9>(plan, a, cur, st);
