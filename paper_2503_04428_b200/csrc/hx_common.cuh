@@ -88,7 +88,7 @@ __device__ __forceinline__ double limited_slope(int lim, double a, double b) {
 // T comes from e (or from P) by Newton-Raphson, as the paper prescribes; started at the smaller of the two
 // single-term roots the iterate can only move down towards the root; it stops when the correction is a few ulp.
 // ---------------------------------------------------------------------------------------------
-__device__ __noinline__ double temperature_root(double a1, double a4, double b) {   // not inlined: keeps the generic kernels small (compile time)   // a1 T + a4 T^4 = b
+static __device__ __noinline__ double temperature_root(double a1, double a4, double b) {   // not inlined: keeps the generic kernels small (compile time)   // a1 T + a4 T^4 = b
   if (!(b > 0.0)) return b / a1;                       // non-physical: a non-positive T makes the caller's P <= 0
   double T = fmin(b / a1, sqrt(sqrt(b / a4)));
   for (int it = 0; it < 60; ++it) {                    // R27: until the correction is a few ulp; quadratic, ~5-9 steps
