@@ -35,35 +35,36 @@ __device__ __forceinline__ int ghost_src(int i, int n, int bc_lo, int bc_hi, boo
 // Work items: three disjoint slab groups that cover the ghost shell --
 //   A: ghost in direction 0, any padded (q1, q2);  B: interior in 0, ghost in 1, any padded q2;  C: interior in 0 and 1, ghost in 2.
 __global__ void ghost_fill_kernel(Layout L, double* __restrict__ U, GhostBC bc) {
-  const int G0 = 2 * L.ng[0], G1 = 2 * L.ng[1], G2 = 2 * L.ng[2];
-  const long long nA = (long long)G0 * L.np[1] * L.np[2];
-  const long long nB = (long long)L.n[0] * G1 * L.np[2];
-  const long long nC = (long long)L.n[0] * L.n[1] * G2;
-  const long long per_field = nA + nB + nC, total = per_field * L.nvar;
-  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
-    const int v = (int)(t / per_field);
-    long long r = t % per_field;
+  // blockIdx.y = field; 32-bit index arithmetic (the shell of one field has far fewer than 2^31 cells: checked by the host)
+  const unsigned G0 = 2 * L.ng[0], G1 = 2 * L.ng[1], G2 = 2 * L.ng[2];
+  const unsigned n0 = L.n[0], n1 = L.n[1], np1 = L.np[1], np2 = L.np[2];
+  const unsigned nA = G0 * np1 * np2, nB = n0 * G1 * np2, nC = n0 * n1 * G2;
+  const unsigned per_field = nA + nB + nC;
+  const int v = blockIdx.y;
+  double* __restrict__ Uv = U + (long long)v * L.sv;
+  for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < per_field; t += gridDim.x * blockDim.x) {
+    unsigned r = t;
     int q[3];   // padded indices of the ghost cell
     if (r < nA) {
-      const int c = (int)(r % G0);
+      const unsigned c = r % G0;
       r /= G0;
-      q[0] = c < L.ng[0] ? c : L.n[0] + c;            // ghosts below: 0..ng-1, above: n+ng..n+2ng-1
-      q[1] = (int)(r % L.np[1]);
-      q[2] = (int)(r / L.np[1]);
+      q[0] = c < (unsigned)L.ng[0] ? c : n0 + c;        // ghosts below: 0..ng-1, above: n+ng..n+2ng-1
+      q[1] = r % np1;
+      q[2] = r / np1;
     } else if (r < nA + nB) {
       r -= nA;
-      q[0] = (int)(r % L.n[0]) + L.ng[0];
-      r /= L.n[0];
-      const int c = (int)(r % G1);
-      q[1] = c < L.ng[1] ? c : L.n[1] + c;
-      q[2] = (int)(r / G1);
+      q[0] = r % n0 + L.ng[0];
+      r /= n0;
+      const unsigned c = r % G1;
+      q[1] = c < (unsigned)L.ng[1] ? c : n1 + c;
+      q[2] = r / G1;
     } else {
       r -= nA + nB;
-      q[0] = (int)(r % L.n[0]) + L.ng[0];
-      r /= L.n[0];
-      q[1] = (int)(r % L.n[1]) + L.ng[1];
-      const int c = (int)(r / L.n[1]);
-      q[2] = c < L.ng[2] ? c : L.n[2] + c;
+      q[0] = r % n0 + L.ng[0];
+      r /= n0;
+      q[1] = r % n1 + L.ng[1];
+      const unsigned c = r / n1;
+      q[2] = c < (unsigned)L.ng[2] ? c : L.n[2] + c;
     }
     int src[3];
     bool neg = false;
@@ -73,8 +74,8 @@ __global__ void ghost_fill_kernel(Layout L, double* __restrict__ U, GhostBC bc) 
       src[d] = ghost_src(q[d] - L.ng[d], L.n[d], bc.lo[d], bc.hi[d], flip) + L.ng[d];
       if (flip && v == 1 + d && d < L.ndim) neg = !neg;
     }
-    const double val = U[v * L.sv + L.off(src[0], src[1], src[2])];
-    U[v * L.sv + L.off(q[0], q[1], q[2])] = neg ? -val : val;
+    const double val = Uv[L.off(src[0], src[1], src[2])];
+    Uv[L.off(q[0], q[1], q[2])] = neg ? -val : val;
   }
 }
 
@@ -85,12 +86,13 @@ cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, cons
     bc.hi[d] = bc_hi[d];
   }
   const long long per_field = 2LL * L.ng[0] * L.np[1] * L.np[2] + 2LL * L.n[0] * L.ng[1] * L.np[2] + 2LL * L.n[0] * L.n[1] * L.ng[2];
-  const long long total = per_field * L.nvar;
-  if (total == 0) return cudaSuccess;
+  if (per_field == 0) return cudaSuccess;
+  if (per_field >= (1LL << 31)) return cudaErrorInvalidValue;   // a ghost shell of 2^31 cells per field would need > 10^13 cells of state
   const int block = 256;
-  long long grid = (total + block - 1) / block;
-  if (grid > 148LL * 32) grid = 148LL * 32;
-  ghost_fill_kernel<<<(unsigned)grid, block, 0, s>>>(L, U, bc);
+  long long gx = (per_field + block - 1) / block;
+  const long long cap = (148LL * 32 + L.nvar - 1) / L.nvar;
+  if (gx > cap) gx = cap;
+  ghost_fill_kernel<<<dim3((unsigned)gx, (unsigned)L.nvar), block, 0, s>>>(L, U, bc);
   return cudaGetLastError();
 }
 
