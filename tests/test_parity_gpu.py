@@ -354,3 +354,21 @@ def test_step_is_deterministic(hx):
             out.append((dts, g.get_state()))
         assert out[0][0] == out[1][0]
         assert np.array_equal(out[0][1], out[1][1])
+
+
+def test_full_size_ten_steps_sedov(hx, oxlib):
+    """Ten steps of config 3 at its full size (256^3) against the whole-array oracle, every cell: L1 relative
+    difference per field <= 1e-9 and max relative difference <= 1e-11 (the blast has crossed a few cells by then)."""
+    ox = oxlib
+    spec, W = wl.sedov_3d(256)
+    g, o = make_pair(hx, ox, spec, W)
+    del W
+    for s in range(10):
+        dt_g, dt_o = g.compute_dt(spec["cfl"]), o.compute_dt(spec["cfl"])
+        assert abs(dt_g - dt_o) <= 1e-11 * dt_o, (s, dt_g, dt_o)
+        g.step(dt_g)
+        o.step(dt_o)
+    assert g.step_kernel == "tile2_uni"
+    Ug, Uo = g.get_state(), o.get_state()
+    assert max(l1_rel_per_field(Ug, Uo, 3)) <= TOL_L1
+    assert max(max_rel_per_field(Ug, Uo, 3)) <= 1e-11
