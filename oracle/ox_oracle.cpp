@@ -3,14 +3,14 @@
 //
 // Plain, slow, whole-array passes in fp64, following PAPER.md in the paper's order:
 //   O0 ghost fill      : Sect. 3.2 "periodic, null gradient, reflective"
-//   O1 cons -> prim    : Eq. 1 + ideal-gas EOS Eq. 5                             (L44-L57, L83-L84)
+//   O1 cons -> prim    : Eq. 1 + ideal-gas EOS Eq. 5, or gas + radiation Eq. 6-7 (L44-L57, L83-L102)
 //   O2 limited slopes  : Eq. 17, limiters Minmod / Van Leer / Van Albada (+ MC)  (L184-L189)
 //   O3 face states     : Eq. 17
 //   O4 Hancock half step: Eq. 18, multi-D as Toro Sect. 16.5 (unsplit)           (L191-L195)
 //   O5 Riemann flux    : HLL / HLLC (Toro 2009)                                  (L197-L201)
-//   O6 update + sources: Eq. 19, spherical sources Eq. 13-16, gravity Eq. 1b-1c, 2, 3
+//   O6 update + sources: Eq. 19, spherical sources Eq. 13-16, gravity Eq. 1b-1c, 2, 3, 4 (self-gravity)
 //   O7 CFL time step   : sum form (reading R2 in DESIGN.md)
-// Where the paper is silent or garbled the readings R1-R25 listed in DESIGN.md apply.
+// Where the paper is silent or garbled the readings R1-R28 listed in DESIGN.md apply.
 //
 // A second, deliberately naive per-cell evaluation (ox_cell_update) is written separately
 // from the same passages with boundary conditions applied by index mapping; tests compare
@@ -19,7 +19,9 @@
 // Shares NO code with the CUDA path.  Compile: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC.
 // Pins: tests/test_oracle_*.py (exact Sod solution, convergence orders, uniform state,
 // conservation, F(U,U)=F(U), stationary contact, symmetry, angular momentum, free fall,
-// spherical 1-D/3-D reduction, Sedov similarity radius, brute force).
+// spherical 1-D/3-D reduction, Sedov similarity radius centred and off-centre, brute force, EOS round trip / Eq. 7
+// against the adiabatic derivative / limits, self-gravity closed forms).  Every function is pinned: none is
+// "parity unpinned".
 #include "ox.h"
 
 #include <algorithm>
