@@ -86,7 +86,11 @@ struct Smem {
   static constexpr int YSTR = (TY + 1) * TX;                   // y-exchange: slots ey = -1 .. TY-1
   static constexpr size_t x_bytes = (size_t)NF * XSTR * sizeof(double);
   static constexpr size_t y_bytes = (size_t)NF * YSTR * sizeof(double);
-  static constexpr size_t fixed = NPL * plane_stride + x_bytes + y_bytes + 64 + 128;
+  // nvar >= 9: the passive-scalar parts of the four predicted states an owner keeps across the first barrier go to
+  // private shared-memory slots instead of registers (the nvar-9 builds spilled them to local memory: long-scoreboard stalls)
+  static constexpr int NPRIV = (NV >= 9) ? 4 * (NV - 5) : 0;
+  static constexpr size_t priv_bytes = (size_t)NPRIV * TY * TX * sizeof(double);
+  static constexpr size_t fixed = NPL * plane_stride + x_bytes + y_bytes + priv_bytes + 64 + 128;
   static constexpr size_t total(int zc) { return fixed + 6 * (size_t)(zc + 6) * sizeof(double); }   // + z tables of one chunk
 };
 
@@ -542,7 +546,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   double* X = (double*)(base + SM::NPL * SM::plane_stride);
   double* Y = X + NF * XSTR;
   uint64_t* mbar = (uint64_t*)(Y + NF * YSTR);
-  double* zt = (double*)(mbar + 8);   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
+  double* priv = (double*)(mbar + 8) + (threadIdx.x & (TY * TX - 1));   // private slots of the owner threads, field stride TY*TX
+  double* zt = (double*)(mbar + 8) + SM::NPRIV * TY * TX;   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
 
   const StepArgs& s = a.s;
   const Layout& L = s.L;
@@ -892,10 +897,18 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           if (lim_none) dUs = 0.0;
           X[(2 + sv) * XSTR + xs_own] = (rf[1] + dUs) * ir6[1];
           Y[(2 + sv) * YSTR + ys_own] = (rf[3] + dUs) * ir6[3];
-          qxm[2 + sv] = (rf[0] + dUs) * ir6[0];
-          qym[2 + sv] = (rf[2] + dUs) * ir6[2];
-          qzm[2 + sv] = (rf[4] + dUs) * ir6[4];
-          zpn[2 + sv] = (rf[5] + dUs) * ir6[5];
+          if (SM::NPRIV > 0) {
+            constexpr int PS = TY * TX;
+            priv[(4 * (sv - 5) + 0) * PS] = (rf[0] + dUs) * ir6[0];
+            priv[(4 * (sv - 5) + 1) * PS] = (rf[2] + dUs) * ir6[2];
+            priv[(4 * (sv - 5) + 2) * PS] = (rf[4] + dUs) * ir6[4];
+            priv[(4 * (sv - 5) + 3) * PS] = (rf[5] + dUs) * ir6[5];
+          } else {
+            qxm[2 + sv] = (rf[0] + dUs) * ir6[0];
+            qym[2 + sv] = (rf[2] + dUs) * ir6[2];
+            qzm[2 + sv] = (rf[4] + dUs) * ir6[4];
+            zpn[2 + sv] = (rf[5] + dUs) * ir6[5];
+          }
           Un[sv] = Wc[0] * fc;
         }
       }
@@ -907,6 +920,16 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       }
       // ======== block 2: the three Riemann problems on the lower faces of this cell (x and y fluxes go back into
       // the slots), finish cell p-1 with the z flux, start cell p =============================================
+      if (SM::NPRIV > 0) {
+        constexpr int PS = TY * TX;
+#pragma unroll
+        for (int sv = 5; sv < NV; ++sv) {
+          qxm[2 + sv] = priv[(4 * (sv - 5) + 0) * PS];
+          qym[2 + sv] = priv[(4 * (sv - 5) + 1) * PS];
+          qzm[2 + sv] = priv[(4 * (sv - 5) + 2) * PS];
+          zpn[2 + sv] = priv[(4 * (sv - 5) + 3) * PS];
+        }
+      }
       double Fx[NV], Fy[NV], Fz[NV];
       {
         double qlx[NF], qly[NF];
