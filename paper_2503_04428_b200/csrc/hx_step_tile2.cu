@@ -53,7 +53,8 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], 
   // the chunk's z tables live in shared memory next to the plane ring and the exchange buffers (227 KB per CTA)
   const size_t plane = ((size_t)L.nvar * (TY + 4) * t2::PX * 8 + 127) / 128 * 128;
   const size_t fixed = 3 * plane + (size_t)(L.nvar + 2) * (TY * (t2::TX + 2) + (TY + 1) * t2::TX) * 8 + 192 +
-                       (L.nvar >= 9 ? (size_t)4 * (L.nvar - 5) * TY * t2::TX * 8 : 0);   // + private scalar slots (nvar >= 9)
+                       (L.nvar >= 9 ? (size_t)4 * (L.nvar - 5) * TY * t2::TX * 8 : 0) +   // + private scalar slots (nvar >= 9)
+                       (size_t)7 * (t2::TX + 2 + TY + 2) * 8;                               // + column / row factor tables
   const size_t budget = 227 * 1024 - 1024;   // static shared memory of the block reduction + reserve
   int nzc = (L.n[2] + 15) / 16;
   double best = -1.0;
