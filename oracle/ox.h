@@ -50,6 +50,7 @@ typedef struct {
   double eos_R;        /* OX_EOS_GAS_RADIATION: k_b / mu (gas constant per unit mass), Eq. 6a     */
   double eos_ar;       /* OX_EOS_GAS_RADIATION: radiation constant a_r, Eq. 6a-6b                 */
   double G;            /* OX_GRAV_SELF: gravitational constant; GM is then G times the central mass M_c */
+  double emon_eps;     /* > 0: internal-energy monitoring (Eq. 10-12) with this epsilon (paper: 1e-6); 0: off */
 } ox_config;
 
 int ox_create(const ox_config* cfg, ox_handle** out);

@@ -278,8 +278,8 @@ double limiter(int lim, double a, double b) {
 
 // O5 Riemann flux between conserved states UL | UR across a face normal to dir (Toro 2009,
 // ch. 10; wave-speed estimates of Davis, reading R14; ties per R15).
-void riemann_flux(int solver, const Eos& eos, int ndim, int nvar, int dir, const double* UL, const double* UR,
-                  double* F) {
+void riemann_flux_core(int solver, const Eos& eos, int ndim, int nvar, int dir, const double* UL, const double* UR,
+                       double* F) {
   double WL[NVMAX], WR[NVMAX], FL[NVMAX], FR[NVMAX];
   cons_to_prim(eos, ndim, nvar, UL, WL);
   cons_to_prim(eos, ndim, nvar, UR, WR);
@@ -323,6 +323,40 @@ void riemann_flux(int solver, const Eos& eos, int ndim, int nvar, int dir, const
   } else {
     for (int v = 0; v < nvar; ++v) F[v] = FR[v];
   }
+}
+
+// Internal-energy monitoring (Eq. 10; reading R29): what the second energy equation
+//   de/dt + div(u e) + P div u = 0
+// needs from a face: the advective flux of e, taken as (mass flux) x (e/rho of the upwind predicted state), and the
+// face velocity "from the standard hydrodynamical step", taken as the contact speed S* of the same Riemann problem
+// (Toro Eq. 10.37 with the wave speeds of R14; the left / right velocity when the whole fan lies on one side).
+void monitor_face(const Eos& eos, int ndim, int nvar, int dir, const double* UL, const double* UR, double Fmass, double& phi,
+                  double& uface) {
+  double WL[NVMAX], WR[NVMAX];
+  cons_to_prim(eos, ndim, nvar, UL, WL);
+  cons_to_prim(eos, ndim, nvar, UR, WR);
+  const int ie = 1 + ndim;
+  const double rL = WL[0], rR = WR[0], uL = WL[1 + dir], uR = WR[1 + dir], PL = WL[ie], PR = WR[ie];
+  const double cL = eos_sound_speed(eos, rL, PL), cR = eos_sound_speed(eos, rR, PR);
+  const double SL = std::min(uL - cL, uR - cR), SR = std::max(uL + cL, uR + cR);
+  if (SL >= 0.0) uface = uL;
+  else if (SR <= 0.0) uface = uR;
+  else {
+    const double mL = rL * (SL - uL), mR = rR * (SR - uR);
+    uface = (PR - PL + uL * mL - uR * mR) / (mL - mR);
+  }
+  const double* UK = (Fmass >= 0.0) ? UL : UR;
+  const double* WK = (Fmass >= 0.0) ? WL : WR;
+  double u2 = 0.0;
+  for (int d = 0; d < ndim; ++d) u2 += WK[1 + d] * WK[1 + d];
+  phi = Fmass * (UK[ie] - 0.5 * WK[0] * u2) / WK[0];
+}
+
+// F[0..nvar-1]: Riemann flux; F[nvar]: advective flux of the internal energy; F[nvar+1]: face velocity (monitoring)
+void riemann_flux(int solver, const Eos& eos, int ndim, int nvar, int dir, const double* UL, const double* UR,
+                  double* F) {
+  riemann_flux_core(solver, eos, ndim, nvar, dir, UL, UR, F);
+  monitor_face(eos, ndim, nvar, dir, UL, UR, F[0], F[nvar], F[nvar + 1]);
 }
 
 // Cell-centred geometric source of the predictor in spherical coordinates (O4, reading R8):
@@ -451,6 +485,32 @@ void update_cell(const ox_handle* h, int i, int j, int k, double dt, const doubl
       Unew[1 + d] = mstar + dt * 0.5 * (Un[0] + Unew[0]) * gd;
       Unew[1 + ndim] += dt * 0.5 * (Un[1 + d] + Unew[1 + d]) * gd;
     }
+  }
+  if (c.emon_eps > 0.0) {   // monitoring of the internal energy in highly supersonic regions (Eq. 10-12, reading R29)
+    const int ie = 1 + ndim;
+    double Wn[NVMAX];
+    cons_to_prim(eos_of(c), ndim, nvar, Un, Wn);
+    double kn = 0.0, k1 = 0.0;
+    for (int d = 0; d < ndim; ++d) {
+      kn += Un[1 + d] * Un[1 + d];
+      k1 += Unew[1 + d] * Unew[1 + d];
+    }
+    const double en = Un[ie] - 0.5 * kn / Un[0];            // e^n
+    const double ek = 0.5 * k1 / Unew[0];                   // kinetic energy of the new state
+    const double e1 = Unew[ie] - ek;                        // e^n + delta^1 e: from the total-energy equation (Eq. 1c)
+    double adv = 0.0, divu = 0.0;                           // Eq. 10: -div(u e) and div u, finite-volume form
+    for (int d = 0; d < ndim; ++d) {
+      adv += Fm[d][nvar] * dS[d][0] - Fp[d][nvar] * dS[d][1];
+      divu += Fp[d][nvar + 1] * dS[d][1] - Fm[d][nvar + 1] * dS[d][0];
+    }
+    const double e2 = en + (dt / dV) * (adv - Wn[ie] * divu);   // e^n + delta^2 e, pressure of the old state
+    const double lim = c.emon_eps * ek;                     // Eq. 12
+    double alpha;
+    if (e1 >= lim) alpha = 1.0;
+    else if (e1 > 0.1 * lim) alpha = (e1 / lim) * (e1 / lim);
+    else alpha = 0.0;
+    const double enew = en + alpha * (e1 - en) + (1.0 - alpha) * (e2 - en);   // Eq. 11
+    Unew[ie] = ek + enew;
   }
 }
 
@@ -817,7 +877,7 @@ int ox_step(ox_handle* h, double dt) {
   // O5: F[d] at cell ci = Riemann flux through the MINUS face of that cell in direction d
   std::vector<double> F[3];
   for (int d = 0; d < ndim; ++d) {
-    F[d].assign((size_t)nvar * ncp, 0.0);
+    F[d].assign((size_t)(nvar + 2) * ncp, 0.0);   // + advective flux of e and face velocity (monitoring)
     int fhi[3] = {c.n[0], c.n[1], c.n[2]};
     fhi[d] += 1;
 #pragma omp parallel for if (h->ncp > 32768)
@@ -833,7 +893,7 @@ int ox_step(ox_handle* h, double dt) {
             UR[v] = Um[d][(size_t)v * ncp + cr];
           }
           riemann_flux(c.riemann, eos_of(c), ndim, nvar, d, UL, UR, Fl);
-          for (int v = 0; v < nvar; ++v) F[d][(size_t)v * ncp + cr] = Fl[v];
+          for (int v = 0; v < nvar + 2; ++v) F[d][(size_t)v * ncp + cr] = Fl[v];
         }
   }
 
@@ -850,7 +910,7 @@ int ox_step(ox_handle* h, double dt) {
           int b[3] = {i, j, k};
           b[d] += 1;
           const size_t cp = h->cell(b[0], b[1], b[2]);
-          for (int v = 0; v < nvar; ++v) {
+          for (int v = 0; v < nvar + 2; ++v) {
             Fm[d][v] = F[d][(size_t)v * ncp + ci];
             Fp[d][v] = F[d][(size_t)v * ncp + cp];
           }
@@ -889,7 +949,7 @@ int ox_cell_update(ox_handle* h, int i, int j, int k, double dt, double* out) {
 int ox_riemann_flux(int riemann, double gamma, int ndim, int ns, int dir, const double* UL, const double* UR,
                     double* F) {
   if (ndim < 1 || ndim > 3 || ns < 0 || 2 + ndim + ns > NVMAX || dir < 0 || dir >= ndim) return OX_ERR_INVALID_ARG;
-  riemann_flux(riemann, gamma, ndim, 2 + ndim + ns, dir, UL, UR, F);
+  riemann_flux_core(riemann, gamma, ndim, 2 + ndim + ns, dir, UL, UR, F);
   return OX_OK;
 }
 

@@ -65,7 +65,7 @@ def centres(faces):
 
 def _spec(name, ndim, n, faces, bc_lo, bc_hi, gamma, limiter, riemann=RIEMANN_HLLC, coords=CARTESIAN,
           n_scalars=0, gravity=GRAV_NONE, g=(0.0, 0.0, 0.0), GM=0.0, cfl=0.8, steps=1, t_end=None, seed=0,
-          eos=EOS_IDEAL, eos_R=0.0, eos_ar=0.0, G=0.0):
+          eos=EOS_IDEAL, eos_R=0.0, eos_ar=0.0, G=0.0, emon_eps=0.0):
     n3 = list(n) + [1] * (3 - len(n))
     return {
         "name": name, "ndim": ndim, "coords": coords, "n": n3,
@@ -76,7 +76,7 @@ def _spec(name, ndim, n, faces, bc_lo, bc_hi, gamma, limiter, riemann=RIEMANN_HL
         "bc_lo": list(bc_lo) + [0] * (3 - len(bc_lo)), "bc_hi": list(bc_hi) + [0] * (3 - len(bc_hi)),
         "eos": eos, "eos_R": eos_R, "eos_ar": eos_ar,
         "gamma": gamma, "riemann": riemann, "limiter": limiter, "n_scalars": n_scalars,
-        "gravity": gravity, "g": list(g), "GM": GM, "G": G,
+        "gravity": gravity, "g": list(g), "GM": GM, "G": G, "emon_eps": emon_eps,
         "cfl": cfl, "steps": steps, "t_end": t_end, "seed": seed,
         "nvar": 2 + ndim + n_scalars,
     }

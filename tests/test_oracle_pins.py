@@ -552,6 +552,10 @@ CASES_P11 = [
     # self-gravity (Eq. 4; gravity code 3): central mass + spherically averaged mass of the grid
     ("s3d_selfgrav", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 3, 1, 1, 1),
     ("s1d_selfgrav", 1, [8], 1, [2], [1], 3, 4, 1, 0),
+    # internal-energy monitoring (Eq. 10-12; names ending in _emon): epsilon = 5 puts cells on all three branches of Eq. 12
+    ("c3d_emon", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 1),
+    ("s3d_emon", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 1),
+    ("c2d_hll_emon", 2, [7, 6], 0, [2, 0], [1, 0], 0, 2, 0, 0),
 ]
 
 
@@ -575,6 +579,8 @@ def random_problem(ox, case, seed=0):
         kw.update(gravity=ox.GRAV_POINT_MASS, GM=0.8)
     elif grav == 3:
         kw.update(gravity=ox.GRAV_SELF, GM=0.8, G=0.6)
+    if name.endswith("_emon"):
+        kw.update(emon_eps=5.0)
     if name.endswith("_rad"):
         kw.update(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0)
     spec = wl._spec(name, ndim, n, faces, bc_lo, bc_hi, 1.4, lim, **kw)
@@ -948,3 +954,60 @@ def test_p13_self_gravity_accelerates_a_static_shell_by_rho_g_dt(oxlib):
     expect = dt * W[0, 0, 0, :] * g
     assert np.max(np.abs(U[1, 1, 1, 1:-1] / expect[1:-1] - 1.0)) <= 1e-3
     assert np.max(np.abs(U[2])) <= 1e-12 and np.max(np.abs(U[3])) <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------ P14: internal-energy monitoring
+def test_p14_monitoring_is_inert_where_the_internal_energy_is_large(oxlib):
+    """Eq. 12: alpha = 1 wherever e >= eps e_k, and then Eq. 11 returns the total-energy result: with eps = 1e-6 a
+    subsonic random problem steps exactly as without monitoring (to the rounding of e_k + (E - e_k))."""
+    ox = oxlib
+    case = ("c3d_mixed", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 2)
+    spec, W = random_problem(ox, case)
+    a, b = make(ox, spec, W), make(ox, dict(spec, emon_eps=1e-6), W)
+    for _ in range(3):
+        dt = a.compute_dt(0.4)
+        a.step(dt)
+        b.step(dt)
+    Ua, Ub = a.get_state(), b.get_state()
+    assert np.max(np.abs(Ua - Ub)) <= 1e-14 * np.max(np.abs(Ua))
+
+
+def test_p14_monitoring_keeps_a_cold_supersonic_stream_cold(oxlib):
+    """The purpose of Eq. 10-12 (L120-L126): a uniform stream with e / e_k = 1e-10.  From the total energy alone the
+    internal energy drifts by rounding of E (relative 1e-16 e_k / e = 1e-6 per step); with monitoring (alpha = 0 there)
+    it follows Eq. 10, whose fluxes cancel exactly in a uniform state."""
+    ox = oxlib
+    spec, W = wl.smooth_periodic(3, [8, 6, 4], seed=2, n_scalars=0, limiter=wl.LIM_MINMOD)
+    W[0], W[1], W[2], W[3], W[4] = 1.3, 3.0e5, -2.0e5, 1.0e5, 2.7
+    drift = {}
+    for eps in (0.0, 1e-6):
+        o = make(ox, dict(spec, emon_eps=eps), W)
+        U0 = o.get_state()
+        e0 = U0[4] - 0.5 * (U0[1] ** 2 + U0[2] ** 2 + U0[3] ** 2) / U0[0]
+        run_steps(o, 0.4, 20)
+        U = o.get_state()
+        e = U[4] - 0.5 * (U[1] ** 2 + U[2] ** 2 + U[3] ** 2) / U[0]
+        drift[eps] = float(np.max(np.abs(e - e0) / e0))
+    assert drift[1e-6] <= 1e-4 * drift[0.0] or drift[1e-6] <= 1e-12, drift
+
+
+def test_p14_second_energy_equation_compression_work(oxlib):
+    """Eq. 10 with uniform rho, e, P and u = a x: de/dt = -(e + P) a.  eps huge puts every cell on the alpha = 0
+    branch; one small step changes e by -(e + P) a dt in the interior (first order in dt and dx)."""
+    ox = oxlib
+    n, a = 64, 0.05
+    fx = wl.uniform_faces(0.0, 1.0, n)
+    spec = wl._spec("emon1d", 1, [n], [fx], [wl.BC_TRANSMISSIVE], [wl.BC_TRANSMISSIVE], 1.4, wl.LIM_MC, emon_eps=1e30)
+    x = 0.5 * (fx[1:] + fx[:-1])
+    W = np.empty((3, 1, 1, n))
+    W[0], W[1, 0, 0], W[2] = 1.0, a * (x - 0.5), 2.0
+    o = make(ox, spec, W)
+    dt = 0.05 * o.compute_dt(0.5)
+    U0 = o.get_state()
+    o.step(dt)
+    U = o.get_state()
+    e0 = U0[2] - 0.5 * U0[1] ** 2 / U0[0]
+    e1 = U[2] - 0.5 * U[1] ** 2 / U[0]
+    got = ((e1 - e0) / dt)[0, 0, 4:-4]
+    want = -(e0[0, 0, 4:-4] + 2.0) * a
+    assert np.max(np.abs(got / want - 1.0)) <= 5e-3, (got[:3], want[:3])
