@@ -67,6 +67,7 @@ typedef struct {
   double eos_R;           /* HX_EOS_GAS_RADIATION: k_b / mu, gas constant per unit mass (Eq. 6a); > 0         */
   double eos_ar;          /* HX_EOS_GAS_RADIATION: radiation constant a_r (Eq. 6a-6b); > 0                    */
   double G;               /* HX_GRAV_SELF: gravitational constant (GM is then G times the central mass)      */
+  double emon_eps;        /* > 0: monitoring of the internal energy (Eq. 10-12) with this epsilon (paper: 1e-6) */
 } hx_config;
 
 /* Validate cfg, allocate the padded double-buffered state and the geometry tables on the current

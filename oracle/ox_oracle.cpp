@@ -8,9 +8,10 @@
 //   O3 face states     : Eq. 17
 //   O4 Hancock half step: Eq. 18, multi-D as Toro Sect. 16.5 (unsplit)           (L191-L195)
 //   O5 Riemann flux    : HLL / HLLC (Toro 2009)                                  (L197-L201)
-//   O6 update + sources: Eq. 19, spherical sources Eq. 13-16, gravity Eq. 1b-1c, 2, 3, 4 (self-gravity)
+//   O6 update + sources: Eq. 19, spherical sources Eq. 13-16, gravity Eq. 1b-1c, 2, 3, 4 (self-gravity),
+//                        internal-energy monitoring Eq. 10-12
 //   O7 CFL time step   : sum form (reading R2 in DESIGN.md)
-// Where the paper is silent or garbled the readings R1-R28 listed in DESIGN.md apply.
+// Where the paper is silent or garbled the readings R1-R29 listed in DESIGN.md apply.
 //
 // A second, deliberately naive per-cell evaluation (ox_cell_update) is written separately
 // from the same passages with boundary conditions applied by index mapping; tests compare

@@ -50,6 +50,7 @@ struct Phys {
   int limiter, riemann, gravity, spherical;
   int eos;                // HX_EOS_IDEAL or HX_EOS_GAS_RADIATION
   double rgas, arad;      // gas + radiation: k_b / mu and the radiation constant a_r (Eq. 6a-6b)
+  double emon_eps;        // > 0: internal-energy monitoring (Eq. 10-12) with this epsilon
 };
 
 struct StepArgs {
@@ -210,6 +211,47 @@ __device__ __forceinline__ void riemann_flux(const Phys& P, int nv, int dir, con
     F[1 + ND] = FK[1 + ND] + SK * (fac * (UK[1 + ND] / rK + (Ss - uK) * (Ss + pK / mK)) - UK[1 + ND]);
     for (int s = 2 + ND; s < nv; ++s) F[s] = FK[s] + SK * (fac * WK[s] - UK[s]);
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Internal-energy monitoring (Eq. 10-12; R29).  Per face, next to the Riemann flux: the advective
+// flux of e = (mass flux) x (e / rho of the upwind predicted state) and the face velocity = contact speed S* of the
+// same Riemann problem (u_L or u_R when the whole fan lies on one side).
+// ---------------------------------------------------------------------------------------------
+template <int ND, int NVA>
+__device__ __forceinline__ void monitor_face(const Phys& P, int nv, int dir, const double* UL, const double* UR, double fmass, double& phi,
+                                             double& uface) {
+  double WL[NVA], WR[NVA];
+  cons_to_prim<ND>(P, nv, UL, WL);
+  cons_to_prim<ND>(P, nv, UR, WR);
+  const double rL = WL[0], rR = WR[0], uL = WL[1 + dir], uR = WR[1 + dir], pL = WL[1 + ND], pR = WR[1 + ND];
+  const double cL = eos_sound_speed(P, rL, pL), cR = eos_sound_speed(P, rR, pR);
+  const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
+  if (SL >= 0.0) {
+    uface = uL;
+  } else if (SR <= 0.0) {
+    uface = uR;
+  } else {
+    const double mL = rL * (SL - uL), mR = rR * (SR - uR);
+    uface = (pR - pL + uL * mL - uR * mR) / (mL - mR);
+  }
+  const bool left = fmass >= 0.0;
+  const double* UK = left ? UL : UR;
+  const double* WK = left ? WL : WR;
+  double u2 = 0.0;
+#pragma unroll
+  for (int d = 0; d < ND; ++d) u2 += WK[1 + d] * WK[1 + d];
+  phi = fmass * (UK[1 + ND] - 0.5 * WK[0] * u2) / WK[0];
+}
+
+// Eq. 11-12: blend of the internal energy e1 (from the total-energy update) and e2 (from Eq. 10); returns the new e.
+__device__ __forceinline__ double monitor_blend(double eps, double en, double e1, double e2, double ek) {
+  const double lim = eps * ek;
+  double alpha;
+  if (e1 >= lim) alpha = 1.0;
+  else if (e1 > 0.1 * lim) alpha = (e1 / lim) * (e1 / lim);
+  else alpha = 0.0;
+  return en + alpha * (e1 - en) + (1.0 - alpha) * (e2 - en);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -93,6 +93,7 @@ const char* check_config(const hx_config* c, int* code) {
   if (c->limiter < HX_LIM_NONE || c->limiter > HX_LIM_MC) return "unknown limiter";
   if (c->n_scalars < 0 || 2 + c->ndim + c->n_scalars > NVMAX) return "too many passive scalars";
   if (c->gravity < HX_GRAV_NONE || c->gravity > HX_GRAV_SELF) return "unknown gravity type";
+  if (!(c->emon_eps >= 0.0)) return "emon_eps must be >= 0";
   if ((c->gravity == HX_GRAV_POINT_MASS || c->gravity == HX_GRAV_SELF) && c->coords != HX_SPHERICAL)
     return "point-mass gravity and self-gravity need spherical coordinates";
   for (int d = 0; d < 3; ++d) {
@@ -364,6 +365,7 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
   h->P.eos = cfg->eos;
   h->P.rgas = cfg->eos_R;
   h->P.arad = cfg->eos_ar;
+  h->P.emon_eps = cfg->emon_eps > 0.0 ? cfg->emon_eps : 0.0;
 
   const size_t bytes = (size_t)L.nvar * (size_t)L.sv * sizeof(double);
   cudaError_t e;

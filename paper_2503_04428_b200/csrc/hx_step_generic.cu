@@ -126,6 +126,8 @@ __global__ void __launch_bounds__(128) step_generic_kernel(StepArgs a) {
     double acc[NVA];
     for (int v = 0; v < nv; ++v) acc[v] = 0.0;
     double FmM[ND][ND], FpM[ND][ND];   // momentum components of the face fluxes (spherical sources)
+    const bool emon = a.P.emon_eps > 0.0;
+    double eadv = 0.0, divu = 0.0;      // Eq. 10 in finite-volume form: -div(u e) and div u from the face quantities
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
       int q[3] = {pidx[0], pidx[1], pidx[2]};
@@ -138,6 +140,12 @@ __global__ void __launch_bounds__(128) step_generic_kernel(StepArgs a) {
       face_state<ND, NVA>(a.P, nv, Wc, sigc[d], hwc, -1.0, dUc, UR);
       riemann_flux<ND, NVA>(a.P, nv, d, UL, UR, F);
       for (int v = 0; v < nv; ++v) acc[v] += F[v] * cm[d];
+      if (emon) {
+        double phi, uf;
+        monitor_face<ND, NVA>(a.P, nv, d, UL, UR, F[0], phi, uf);
+        eadv += phi * cm[d];
+        divu -= uf * cm[d];
+      }
 #pragma unroll
       for (int e = 0; e < ND; ++e) FmM[d][e] = F[1 + e];
       // plus face: own plus state | neighbour's minus state
@@ -147,6 +155,12 @@ __global__ void __launch_bounds__(128) step_generic_kernel(StepArgs a) {
       face_state<ND, NVA>(a.P, nv, Wn, sign[d], a.T.hw[d][q[d]], -1.0, dUn, UR);
       riemann_flux<ND, NVA>(a.P, nv, d, UL, UR, F);
       for (int v = 0; v < nv; ++v) acc[v] -= F[v] * cp[d];
+      if (emon) {
+        double phi, uf;
+        monitor_face<ND, NVA>(a.P, nv, d, UL, UR, F[0], phi, uf);
+        eadv -= phi * cp[d];
+        divu += uf * cp[d];
+      }
 #pragma unroll
       for (int e = 0; e < ND; ++e) FpM[d][e] = F[1 + e];
     }
@@ -177,6 +191,18 @@ __global__ void __launch_bounds__(128) step_generic_kernel(StepArgs a) {
         Unew[1 + ND] += a.dt * 0.5 * (Un[1 + d] + mnew) * g;
         Unew[1 + d] = mnew;
       }
+    }
+    if (emon) {   // Eq. 11-12: e^{n+1} from the blend, E reset to e_k + e (R29)
+      double kn = 0.0, k1 = 0.0;
+#pragma unroll
+      for (int d = 0; d < ND; ++d) {
+        kn += Un[1 + d] * Un[1 + d];
+        k1 += Unew[1 + d] * Unew[1 + d];
+      }
+      const double en = Un[1 + ND] - 0.5 * kn / Un[0], ek = 0.5 * k1 / Unew[0];
+      const double e1 = Unew[1 + ND] - ek;
+      const double e2 = en + a.dt * (eadv - Wc[1 + ND] * divu);
+      Unew[1 + ND] = ek + monitor_blend(a.P.emon_eps, en, e1, e2, ek);
     }
     for (int v = 0; v < nv; ++v) a.Uout[v * L.sv + o] = Unew[v];
 

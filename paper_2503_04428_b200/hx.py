@@ -39,7 +39,7 @@ class HxConfig(C.Structure):
         ("eos", C.c_int), ("gamma", C.c_double),
         ("riemann", C.c_int), ("limiter", C.c_int), ("n_scalars", C.c_int),
         ("gravity", C.c_int), ("g", C.c_double * 3), ("GM", C.c_double),
-        ("eos_R", C.c_double), ("eos_ar", C.c_double), ("G", C.c_double),
+        ("eos_R", C.c_double), ("eos_ar", C.c_double), ("G", C.c_double), ("emon_eps", C.c_double),
     ]
 
 
@@ -112,6 +112,7 @@ def make_config(spec: dict):
     cfg.eos_R = float(spec.get("eos_R", 0.0))
     cfg.eos_ar = float(spec.get("eos_ar", 0.0))
     cfg.G = float(spec.get("G", 0.0))
+    cfg.emon_eps = float(spec.get("emon_eps", 0.0))
     cfg.gamma = float(spec["gamma"])
     cfg.riemann = int(spec.get("riemann", RIEMANN_HLLC))
     cfg.limiter = int(spec.get("limiter", LIM_MINMOD))

@@ -239,6 +239,25 @@ def wedge_3d_selfgrav(n=(1024, 256, 256), seed=1005):
     return spec, W
 
 
+def cold_stream_3d(n=256, seed=1006):
+    """a workload for the monitoring of the internal energy in highly supersonic regions (PAPER.md
+    Eq. 10-12): a cold stream, Mach ~ 2800, crossing a periodic unit box with 20 % density and 10 % pressure
+    structure and 0.01 % seeded velocity noise (0.3, subsonic in the stream frame); e / e_k ~ 4e-7, so that with the paper's epsilon = 1e-6 the cells sit on the
+    blended branch of Eq. 12 (alpha ~ 0.1-0.2).  gamma = 1.4, MC + HLLC, CFL 0.6, 50 steps."""
+    nx, ny, nz = (n, n, n) if np.isscalar(n) else n
+    fs = [uniform_faces(0.0, 1.0, m) for m in (nx, ny, nz)]
+    spec = _spec("cold_stream_3d", 3, [nx, ny, nz], fs, [BC_PERIODIC] * 3, [BC_PERIODIC] * 3, 1.4, LIM_MC, cfl=0.6, steps=50,
+                 seed=seed, emon_eps=1e-6)
+    x, y, z = centres(fs[0])[None, None, :], centres(fs[1])[None, :, None], centres(fs[2])[:, None, None]
+    W = np.empty((5, nz, ny, nx))
+    W[0] = 1.0 + 0.2 * np.sin(2 * math.pi * x) * np.cos(2 * math.pi * y) + 0.0 * z
+    W[1] = 3000.0 * (1.0 + 1e-4 * noise(seed, (nz, ny, nx)))
+    W[2] = -2000.0
+    W[3] = 1000.0
+    W[4] = 1.0 + 0.1 * np.cos(2 * math.pi * z) * np.sin(2 * math.pi * x) + 0.0 * y
+    return spec, W
+
+
 CONFIGS = {"sod_1d": sod_1d, "kh_2d": kh_2d, "sedov_3d": sedov_3d, "rt_3d": rt_3d, "wedge_3d": wedge_3d}
 
 

@@ -29,9 +29,9 @@ def test_library_loads_and_exports_every_declared_symbol():
 
 def test_config_struct_matches_header_layout():
     # 3 ints, 6 doubles, 3 ints, 3 pointers, 6 ints, int + double, 3 ints, int, 3 doubles, double, 2 doubles (EOS constants)
-    assert C.sizeof(hx.HxConfig) == 224
+    assert C.sizeof(hx.HxConfig) == 232
     assert hx.HxConfig.faces.offset == 88 and hx.HxConfig.gamma.offset == 144 and hx.HxConfig.GM.offset == 192
-    assert hx.HxConfig.eos_R.offset == 200 and hx.HxConfig.eos_ar.offset == 208 and hx.HxConfig.G.offset == 216
+    assert hx.HxConfig.eos_R.offset == 200 and hx.HxConfig.eos_ar.offset == 208 and hx.HxConfig.G.offset == 216 and hx.HxConfig.emon_eps.offset == 224
 
 
 def test_invalid_arguments_rejected_without_gpu():
