@@ -42,7 +42,7 @@ WORKLOADS = {
     "sedov_wedge_3d": (lambda: wl.sedov_wedge_3d(256), lambda: wl.sedov_wedge_3d(64)),   # PAPER.md Sect. 4.3
     "wedge_3d_rad": (lambda: wl.wedge_3d_rad((1024, 256, 256)), lambda: wl.wedge_3d_rad((96, 24, 24))),   # Eq. 6-7
     "wedge_3d_selfgrav": (lambda: wl.wedge_3d_selfgrav((1024, 256, 256)), lambda: wl.wedge_3d_selfgrav((192, 48, 48))),   # Eq. 4
-    "cold_stream_3d": (lambda: wl.cold_stream_3d(256), lambda: wl.cold_stream_3d(64)),   # Eq. 10-12 (generic kernel)
+    "cold_stream_3d": (lambda: wl.cold_stream_3d(256), lambda: wl.cold_stream_3d(64)),   # Eq. 10-12
     "kh_2d": (lambda: wl.kh_2d(1024), lambda: wl.kh_2d(512)),
     "sod_1d": (lambda: wl.sod_1d(1000), lambda: wl.sod_1d(1000)),
     # small case for quick checks of this script

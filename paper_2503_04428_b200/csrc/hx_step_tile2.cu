@@ -26,7 +26,9 @@ static EncodeTiledFn get_encode_fn() {
 static bool nv_supported(int nv) { return nv == 5 || nv == 6 || nv == 7 || nv == 9; }
 
 int tile2_supported(const Layout& L, const Phys& P) {
-  if (P.emon_eps > 0.0) return 0;   // internal-energy monitoring (Eq. 10-12): generic kernel only so far
+  if (P.emon_eps > 0.0 && !(L.nvar == 5 && !P.spherical && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MC && P.riemann == HX_RIEMANN_HLLC &&
+                            P.eos == HX_EOS_IDEAL))
+    return 0;   // internal-energy monitoring (Eq. 10-12): one tile instantiation (cold_stream_3d), else the generic kernel
   if (P.eos != HX_EOS_IDEAL && L.nvar != 9) return 0;   // gas + radiation EOS: tile kernel instantiated for nvar 9 only, else generic
   return L.ndim == 3 && nv_supported(L.nvar) && L.n[0] >= 2 && L.n[1] >= 2 && L.n[2] >= 2;
 }

@@ -523,6 +523,31 @@ __device__ __forceinline__ void hllc_n(const int (&dir)[N], const double* const*
   }
 }
 
+// Internal-energy monitoring (Eq. 10-12, R29; EMON instantiations): per face, from the two records and the
+// mass flux of the Riemann solution, the advective flux of e (mass flux x e/rho of the upwind state) and the face
+// velocity (contact speed S*, or u_L / u_R when the fan lies on one side).
+template <int DIR>
+__device__ __forceinline__ void monitor_rec(const double* L, const double* R, double fmass, double& phi, double& uf) {
+  const double uL = L[1 + DIR], uR = R[1 + DIR];
+  const double SL = dmin(uL - L[6], uR - R[6]), SR = dmax(uL + L[6], uR + R[6]);
+  const double mL = L[0] * (SL - uL), mR = R[0] * (SR - uR);
+  const double Ss = (R[4] - L[4] + uL * mL - uR * mR) * rcp3(mL - mR);
+  uf = (SL >= 0.0) ? uL : ((SR <= 0.0) ? uR : Ss);
+  const bool left = fmass >= 0.0;
+  const double r = left ? L[0] : R[0], E = left ? L[5] : R[5];
+  const double u1 = left ? L[1] : R[1], u2 = left ? L[2] : R[2], u3 = left ? L[3] : R[3];
+  phi = fmass * fma(-0.5 * r, fma(u3, u3, fma(u2, u2, u1 * u1)), E) * rcp3(r);
+}
+
+__device__ __forceinline__ double monitor_blend2(double eps, double en, double e1, double e2, double ek) {   // Eq. 11-12
+  const double lim = eps * ek;
+  double alpha;
+  if (e1 >= lim) alpha = 1.0;
+  else if (e1 > 0.1 * lim) alpha = (e1 * rcp3(lim)) * (e1 * rcp3(lim));
+  else alpha = 0.0;
+  return en + alpha * (e1 - en) + (1.0 - alpha) * (e2 - en);
+}
+
 // ------------------------------------------------------------------------------------------------
 // The kernel.  Thread roles (warp-uniform except in the last warp):
 //   warps 0..TY-1  owners of row ey = warp, cell ex = lane
@@ -534,7 +559,7 @@ __device__ __forceinline__ void hllc_n(const int (&dir)[N], const double* const*
 // setmaxnreg: the ring path needs far fewer registers than it is given at launch, and ptxas interleaves the
 // independent fp64 chains of the owner path only when it has ~200 registers (at 168 it emits them serially).
 // ------------------------------------------------------------------------------------------------
-template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int TY, int EOS = HX_EOS_IDEAL>
+template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int TY, int EOS = HX_EOS_IDEAL, bool EMON = false>
 __global__ void __launch_bounds__((TY + 4) * 32, 1)
 step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Args a) {
   static_assert(TY % 4 == 0 && TY >= 4 && TY <= 32, "owner warps must fill whole warpgroups (setmaxnreg)");
@@ -742,6 +767,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   double Un0 = 0.0, Unm[3] = {0.0, 0.0, 0.0};   // rho^n, m^n of the previous plane (time-centred gravity)
   double Ul[5] = {1.0, 0.0, 0.0, 0.0, 1.0};     // rho, m, E of the cell written one iteration ago (deferred CFL rate)
   bool st_l = false;                            // ... and whether it was stored
+  double EA = 0.0, DV = 0.0, en_p = 1.0, Pn_p = 1.0;   // EMON: dt x (-div(u e)) and dt x div u of the previous plane's cell so far; its e^n, P^n
   double rate_max = 0.0;
   bool bad = false;
 #pragma unroll
@@ -897,6 +923,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         Un[3] = rho * Wc[3];
         Un[4] = fma(0.5, fma(Un[3], Wc[3], fma(Un[2], Wc[2], Un[1] * Wc[1])), EOS == HX_EOS_IDEAL ? Wc[4] * P.igm1 : ec);
       }
+      const double Pn_c = Wc[4], en_c = (EOS == HX_EOS_IDEAL) ? Wc[4] * P.igm1 : ec;   // EMON: P^n, e^n of cell p
       if constexpr (NV > 5) {
         // Passive scalars one at a time (R7: mass fractions are reconstructed, rho f is advanced): limited slopes,
         // the six face values, the scalar's own half-step increment from the face mass fluxes kept in `unc`, and
@@ -966,6 +993,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         }
       }
       double Fx[NV], Fy[NV], Fz[NV];
+      double phx = 0.0, ufx = 0.0, phy = 0.0, ufy = 0.0, phz = 0.0, ufz = 0.0;
       {
         double qlx[NF], qly[NF];
 #pragma unroll
@@ -988,6 +1016,15 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         for (int v = 0; v < NV; ++v) {
           X[v * XSTR + xs_nbr] = Fx[v];
           Y[v * YSTR + ys_nbr] = Fy[v];
+        }
+        if (EMON) {   // Eq. 10: advective flux of e and face velocity of the three lower faces; x and y ones ride in the two spare slot fields
+          monitor_rec<0>(qlx, qxm, Fx[0], phx, ufx);
+          monitor_rec<1>(qly, qym, Fy[0], phy, ufy);
+          monitor_rec<2>(zp, qzm, Fz[0], phz, ufz);
+          X[NV * XSTR + xs_nbr] = phx;
+          X[(NV + 1) * XSTR + xs_nbr] = ufx;
+          Y[NV * YSTR + ys_nbr] = phy;
+          Y[(NV + 1) * YSTR + ys_nbr] = ufy;
         }
       }
 #pragma unroll
@@ -1013,6 +1050,12 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           const double m3 = fma(rs, hgzp, Unew[3]);
           Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
           Unew[3] = m3;
+        }
+        if (EMON) {   // Eq. 11-12 for cell p-1: e1 from the total energy, e2 from Eq. 10 (dt folded into the coefficients), E reset
+          const double eaf = fma(-k2p, phz, EA), dvf = fma(k2p, ufz, DV);
+          const double ek = 0.5 * fma(Unew[3], Unew[3], fma(Unew[2], Unew[2], Unew[1] * Unew[1])) * rcp3(Unew[0]);
+          const double e1 = Unew[4] - ek, e2 = en_p + fma(-Pn_p, dvf, eaf);
+          Unew[4] = ek + monitor_blend2(P.emon_eps, en_p, e1, e2, ek);
         }
         st_l = st_ok && (p > k0);
         if (st_l) {
@@ -1045,6 +1088,12 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Unm[1] = Un[2];
           Unm[2] = Un[3];
         }
+        if (EMON) {
+          EA = fma(k2m, phz, fma(K.m0, phx, K.m1 * phy));
+          DV = -fma(k2m, ufz, fma(K.m0, ufx, K.m1 * ufy));
+          en_p = en_c;
+          Pn_p = Pn_c;
+        }
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (2) fluxes visible
       // ======== block 3: fluxes through the upper x and y faces come back in the own slots ================
@@ -1053,6 +1102,10 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       Kp.xp = GTAB ? GX(3) : kxp;
       Kp.p1 = GTAB ? GX(4) * GY(1) : k1p;
       Kp.yp = GTAB ? GX(4) * GY(3) : kyp;
+      if (EMON) {
+        EA -= fma(Kp.p0, X[NV * XSTR + xs_own], Kp.p1 * Y[NV * YSTR + ys_own]);
+        DV += fma(Kp.p0, X[(NV + 1) * XSTR + xs_own], Kp.p1 * Y[(NV + 1) * YSTR + ys_own]);
+      }
 #pragma unroll
       for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? Kp.xp : Kp.p0), X[v * XSTR + xs_own], Up[v]);
       if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
@@ -1086,6 +1139,12 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         riemann_fs<NV, RS, 1>(P, ql, q, F);
 #pragma unroll
         for (int v = 0; v < NV; ++v) Y[v * YSTR + ys_nbr] = F[v];
+        if (EMON) {
+          double ph, uf;
+          monitor_rec<1>(ql, q, F[0], ph, uf);
+          Y[NV * YSTR + ys_nbr] = ph;
+          Y[(NV + 1) * YSTR + ys_nbr] = uf;
+        }
       } else if (wid == TY + 3 && act) {
         double ql[NF], F[NV];
 #pragma unroll
@@ -1093,6 +1152,12 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         riemann_fs<NV, RS, 0>(P, ql, q, F);
 #pragma unroll
         for (int v = 0; v < NV; ++v) X[v * XSTR + xs_nbr] = F[v];
+        if (EMON) {
+          double ph, uf;
+          monitor_rec<0>(ql, q, F[0], ph, uf);
+          X[NV * XSTR + xs_nbr] = ph;
+          X[(NV + 1) * XSTR + xs_nbr] = uf;
+        }
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (2)
     }

@@ -19,10 +19,10 @@ struct Plan {
 template <int NV>
 cudaError_t launch_nv(Plan& plan, const Args& a, int cur, cudaStream_t st);
 
-template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EOS_IDEAL>
+template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EOS_IDEAL, bool EMON = false>
 static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   constexpr int TY = TY_DEFAULT;
-  auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY, EOS>;
+  auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY, EOS, EMON>;
   const size_t smem = Smem<NV, TY>::total(plan.zc);
   static size_t attr_set = 0;
   if (attr_set < smem) {
@@ -30,7 +30,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t s
     if (e != cudaSuccess) return e;
     attr_set = smem;
   }
-  plan.name = UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad");
+  plan.name = EMON ? "tile2_emon" : (UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
   kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();
 }

@@ -235,6 +235,7 @@ def test_tile_edges(hx, oxlib, n):
 UNIFORM = {   # 2^k cells on dyadic extents: bitwise-uniform tables -> the constant-geometry instantiations
     "sedov_3d": lambda: wl.sedov_3d((64, 32, 32)),
     "rt_3d": lambda: wl.rt_3d((32, 64, 64)),
+    "cold_stream_3d": lambda: wl.cold_stream_3d((64, 32, 32)),   # internal-energy monitoring in the tile kernel
 }
 
 
@@ -249,7 +250,7 @@ def test_uniform_grid_instantiations(hx, oxlib, name):
         g.step(dt_g)
         o.step(dt_o)
         if s == 0:
-            assert g.step_kernel == "tile2_uni"
+            assert g.step_kernel == ("tile2_emon" if name == "cold_stream_3d" else "tile2_uni")
             rel = max_rel_per_field(g.get_state(), o.get_state(), 3)
             assert max(rel) <= TOL_STEP, (name, rel)
     l1 = l1_rel_per_field(g.get_state(), o.get_state(), 3)
