@@ -23,10 +23,10 @@
 //   * keeps geometry out of registers on bitwise-uniform Cartesian grids (UNI: kernel-parameter constants), and
 //     as per-thread / per-plane 1-D table products otherwise;
 //   * is instantiated for the ideal gas (Eq. 5) and, for nvar 9, for the gas + radiation EOS (Eq. 6-7, Newton-
-//     Raphson for T inside the kernel).
+//     Raphson for T inside the kernel); one instantiation carries the internal-energy monitoring of Eq. 10-12 (EMON).
 //
 // PAPER.md: Eq. 17 (slopes), Eq. 18 + Toro 16.5 (unsplit predictor), Eq. 19 (update), L201 (HLL/HLLC),
-// Eq. 13-16 (spherical sources), Eq. 2-3 (gravity), Eq. 5-7 (EOS); readings R1-R27.
+// Eq. 13-16 (spherical sources), Eq. 2-4 (gravity), Eq. 5-7 (EOS), Eq. 10-12 (monitoring); readings R1-R29.
 #pragma once
 #include <cuda.h>
 
