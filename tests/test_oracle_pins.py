@@ -1011,3 +1011,113 @@ def test_p14_second_energy_equation_compression_work(oxlib):
     got = ((e1 - e0) / dt)[0, 0, 4:-4]
     want = -(e0[0, 0, 4:-4] + 2.0) * a
     assert np.max(np.abs(got / want - 1.0)) <= 5e-3, (got[:3], want[:3])
+
+
+# ---- P14b: the one-sided (supersonic) branches of the face velocity and the upwind choice of the advective flux of e ----
+def _supersonic_tube(n, sign, limiter, eps, rho, u, e, gamma=1.4):
+    """1-D tube, transmissive faces, primitive fields rho(x), sign * u(x), P = (gamma - 1) e(x)."""
+    fx = wl.uniform_faces(0.0, 1.0, n)
+    spec = wl._spec("emon_super", 1, [n], [fx], [wl.BC_TRANSMISSIVE], [wl.BC_TRANSMISSIVE], gamma, limiter, emon_eps=eps)
+    x = wl.centres(fx)
+    if sign < 0:
+        x = 1.0 - x            # the mirror image of the sign > 0 problem
+    W = np.empty((3, 1, 1, n))
+    W[0, 0, 0], W[1, 0, 0], W[2, 0, 0] = rho(x), sign * u(x), (gamma - 1.0) * e(x)
+    return spec, W, fx
+
+
+def _internal_energy_1d(U):
+    return (U[2] - 0.5 * U[1] ** 2 / U[0])[0, 0]
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_p14_supersonic_faces_take_everything_from_upstream(oxlib, sign):
+    """Eq. 10-12 where the whole Riemann fan lies on one side (S_L >= 0, resp. S_R <= 0): the flux is the upstream flux,
+    so with first-order states (limiter NONE) no cell may depend on anything downstream of it -- neither through the
+    face velocity of Eq. 10 (u_L, resp. u_R) nor through the advected e (upwind by the sign of the mass flux).  Two
+    runs that differ only downstream of x = 0.5 (velocity, density, internal energy: all still supersonic) must agree
+    BITWISE upstream of it; eps huge puts every cell on the alpha = 0 branch so that e comes from Eq. 10 alone.
+    Taking u_R for u_L, or the downstream e, changes the last upstream cell."""
+    ox = oxlib
+    n = 48
+
+    def run(downstream):
+        du, dr, de = downstream
+        spec, W, _ = _supersonic_tube(n, sign, wl.LIM_NONE, 1e30,
+                                      lambda x: 1.0 + dr * (x > 0.5), lambda x: 40.0 + du * (x > 0.5),
+                                      lambda x: 2.0 + 0.3 * np.sin(7.0 * x) + de * (x > 0.5))
+        o = make(ox, spec, W)
+        dt = 0.3 / (n * 60.0)
+        for _ in range(3):
+            o.step(dt)
+        return o.get_state()
+
+    Ua, Ub = run((0.0, 0.0, 0.0)), run((9.0, 0.7, 1.1))
+    up = slice(0, n // 2 - 3) if sign > 0 else slice(n // 2 + 3, n)   # three steps move information by three cells at most
+    down = slice(n // 2 + 1, n) if sign > 0 else slice(0, n // 2 - 1)
+    assert np.array_equal(Ua[:, 0, 0, up], Ub[:, 0, 0, up])
+    assert np.max(np.abs(Ua[:, 0, 0, down] - Ub[:, 0, 0, down])) > 0.1
+    # one step: only the cell adjacent to the jump could see it, and it must not
+    spec, W, _ = _supersonic_tube(n, sign, wl.LIM_NONE, 1e30, lambda x: 1.0 + 0.7 * (x > 0.5), lambda x: 40.0 + 9.0 * (x > 0.5),
+                                  lambda x: 2.0 + 1.1 * (x > 0.5))
+    spec0, W0, _ = _supersonic_tube(n, sign, wl.LIM_NONE, 1e30, lambda x: 1.0 + 0.0 * x, lambda x: 40.0 + 0.0 * x, lambda x: 2.0 + 0.0 * x)
+    a, b = make(ox, spec, W), make(ox, spec0, W0)
+    a.step(1e-4)
+    b.step(1e-4)
+    last_up = n // 2 - 1 if sign > 0 else n // 2
+    assert np.array_equal(a.get_state()[:, 0, 0, last_up], b.get_state()[:, 0, 0, last_up])
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_p14_supersonic_advection_of_e_is_first_order_upwind(oxlib, sign):
+    """Uniform rho and u = sign * u0 with u0 > c everywhere, e(x) not uniform, limiter NONE, alpha = 0: div u = 0 at every
+    face (u_f = u_L = u0, resp. u_R), the mass flux is rho u0, so Eq. 10 reduces to the donor-cell update
+    e_i <- e_i - (u0 dt / dx) (e_i - e_upstream) -- a closed form that a downstream-biased Phi, a wrong sign of the
+    flux difference or a non-zero compression term would miss at O(1)."""
+    ox = oxlib
+    n, u0 = 64, 30.0
+    prof = lambda x: 2.0 + 0.8 * np.sin(2.0 * np.pi * x) + 0.3 * (x > 0.4)
+    spec, W, fx = _supersonic_tube(n, sign, wl.LIM_NONE, 1e30, lambda x: 1.7 + 0.0 * x, lambda x: u0 + 0.0 * x, prof)
+    o = make(ox, spec, W)
+    U0 = o.get_state()
+    dt, dx = 0.4 / (n * (u0 + 2.0)), 1.0 / n
+    o.step(dt)
+    e0, e1 = _internal_energy_1d(U0), _internal_energy_1d(o.get_state())
+    up = np.roll(e0, 1) if sign > 0 else np.roll(e0, -1)
+    want = e0 - (u0 * dt / dx) * (e0 - up)
+    inner = slice(2, n - 2)
+    # e is recovered from E - e_k with e_k / e ~ 400: rounding 400 x 1e-16
+    assert np.max(np.abs(e1[inner] - want[inner]) / want[inner]) <= 1e-12
+    # and the total-energy route does NOT give this (the pressure gradient does work on the stream; 1e-7 here): the pin is not vacuous
+    spec_off = dict(spec, emon_eps=0.0)
+    p = make(ox, spec_off, W)
+    p.step(dt)
+    e_plain = _internal_energy_1d(p.get_state())
+    assert np.max(np.abs(e_plain[inner] - want[inner]) / want[inner]) > 1e-8
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_p14_supersonic_compression_work_uses_the_upstream_face_velocity(oxlib, sign):
+    """Uniform rho, e, P, supersonic u = sign * (u0 + b (x - 1/2)^2), limiter NONE, alpha = 0.  With u_f the UPSTREAM state's
+    velocity, Eq. 10 gives e_i <- e_i - dt (e + P) (u_i - u_{i-1}) / dx (backward difference for sign > 0, its mirror
+    image for sign < 0); the downstream state's velocity would give the forward difference, which differs by
+    2 b dx (e + P) dt -- four orders above the tolerance."""
+    ox = oxlib
+    n, u0, b, gamma = 64, 30.0, 6.0, 1.4
+    e_c = 2.0
+    spec, W, fx = _supersonic_tube(n, sign, wl.LIM_NONE, 1e30, lambda x: 1.0 + 0.0 * x, lambda x: u0 + b * (x - 0.5) ** 2, lambda x: e_c + 0.0 * x)
+    o = make(ox, spec, W)
+    U0 = o.get_state()
+    dt, dx = 0.2 / (n * (u0 + 4.0)), 1.0 / n
+    o.step(dt)
+    e1 = _internal_energy_1d(o.get_state())
+    u = W[1, 0, 0]
+    du_up = (u - np.roll(u, 1)) / dx if sign > 0 else (np.roll(u, -1) - u) / dx
+    du_down = (np.roll(u, -1) - u) / dx if sign > 0 else (u - np.roll(u, 1)) / dx
+    P = (gamma - 1.0) * e_c
+    want = e_c - dt * (e_c + P) * du_up
+    wrong = e_c - dt * (e_c + P) * du_down
+    inner = slice(2, n - 2)
+    tol = 2e-13 * 500.0          # rounding of E - e_k with e_k / e ~ 250
+    assert np.max(np.abs(e1[inner] - want[inner])) <= tol * e_c
+    assert np.min(np.abs(wrong[inner] - want[inner])) >= 1e3 * tol * e_c
