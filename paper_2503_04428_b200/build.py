@@ -9,7 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
-LIB = os.path.join(HERE, "libhx.so")
+# HX_LIBRARY: load (and build into) another file, e.g. an A/B variant built with other -D flags
+LIB = os.environ.get("HX_LIBRARY") or os.path.join(HERE, "libhx.so")
 SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_probe.cu",
            "hx_step_tile2.cu", "hx_step_tile2_nv5.cu", "hx_step_tile2_nv6.cu", "hx_step_tile2_nv7.cu", "hx_step_tile2_nv9.cu", "hx_step_tile2_nv9_rad.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -21,15 +22,19 @@ def _deps():
     return max(os.path.getmtime(p) for p in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps():
-        return LIB
+def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str = None, objdir: str = None) -> str:
+    """extra_flags / lib / objdir: variant builds (other -D flags into another .so, objects kept apart)."""
+    lib = lib or LIB
+    objdir = objdir or CSRC
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= _deps():
+        return lib
+    os.makedirs(objdir, exist_ok=True)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
     for src in SOURCES:
-        obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     for src, p in procs:
@@ -38,9 +43,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out)
         if p.returncode != 0:
             raise RuntimeError(f"nvcc failed on {src}")
-    cmd = [nvcc, "-shared", "-o", LIB] + objs + ["-lcudart", "-lcuda"]
+    cmd = [nvcc, "-shared", "-o", lib] + objs + ["-lcudart", "-lcuda"]
     subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 def ensure() -> str:

@@ -23,6 +23,17 @@ static EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
+static size_t smem_fixed(int nv) {   // shared memory of one CTA without the z tables of its chunk
+  constexpr int TY = t2::TY_DEFAULT;
+  switch (nv) {
+    case 5: return t2::Smem<5, TY>::fixed;
+    case 6: return t2::Smem<6, TY>::fixed;
+    case 7: return t2::Smem<7, TY>::fixed;
+    case 9: return t2::Smem<9, TY>::fixed;
+    default: return 0;
+  }
+}
+
 static bool nv_supported(int nv) { return nv == 5 || nv == 6 || nv == 7 || nv == 9; }
 
 int tile2_supported(const Layout& L, const Phys& P) {
@@ -54,10 +65,7 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], 
   }
   const long long cols = (long long)ntx * nty;
   // the chunk's z tables live in shared memory next to the plane ring and the exchange buffers (227 KB per CTA)
-  const size_t plane = ((size_t)L.nvar * (TY + 4) * t2::PX * 8 + 127) / 128 * 128;
-  const size_t fixed = 3 * plane + (size_t)(L.nvar + 2) * (TY * (t2::TX + 2) + (TY + 1) * t2::TX) * 8 + 192 +
-                       (L.nvar >= 9 ? (size_t)4 * (L.nvar - 5) * TY * t2::TX * 8 : 0) +   // + private scalar slots (nvar >= 9)
-                       (size_t)7 * (t2::TX + 2 + TY + 2) * 8;                               // + column / row factor tables
+  const size_t fixed = smem_fixed(L.nvar);
   const size_t budget = 227 * 1024 - 1024;   // static shared memory of the block reduction + reserve
   int nzc = (L.n[2] + 15) / 16;
   double best = -1.0;

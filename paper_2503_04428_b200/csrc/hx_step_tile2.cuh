@@ -73,8 +73,18 @@ struct Args {
   double uil[3];     // 1 / delta_d  (CFL inverse lengths)
 };
 
+// One CTA-wide barrier per plane instead of two: the exchange slots are double buffered by plane parity, so the flux a
+// neighbour writes back into a slot during plane p is picked up after the barrier of plane p+1 while the "+" states
+// of plane p+1 already sit in the other buffer.  Needs twice the slot memory: field counts whose buffers fit.
+#ifndef HX_T2_ONEBAR
+#define HX_T2_ONEBAR 1
+#endif
+constexpr bool one_barrier(int nv) { return HX_T2_ONEBAR && nv <= 8; }
+
 template <int NV, int TY>
 struct Smem {
+  static constexpr bool ONEBAR = one_barrier(NV);
+  static constexpr int NXY = ONEBAR ? 2 : 1;
   static constexpr int PY = TY + 4;
   static constexpr int NF = NV + 2;
   static constexpr int FSTR = PY * PX;                         // field stride inside a plane (doubles)
@@ -93,7 +103,8 @@ struct Smem {
   // spherical builds: 1-D factors of the update / CFL coefficients by tile column and tile row (7 + 7 tables), so that
   // their per-thread products need no registers (they used to be spilled: 20 doubles per thread)
   static constexpr int GT_X = TX + 2, GT_Y = TY + 2, GT_N = 7 * (GT_X + GT_Y);
-  static constexpr size_t fixed = NPL * plane_stride + x_bytes + y_bytes + priv_bytes + GT_N * sizeof(double) + 64 + 128;
+  static constexpr int XYSTR = NF * (XSTR + YSTR);             // doubles of one parity buffer (X fields, then Y fields)
+  static constexpr size_t fixed = NPL * plane_stride + NXY * (x_bytes + y_bytes) + priv_bytes + GT_N * sizeof(double) + 64 + 128;
   static constexpr size_t total(int zc) { return fixed + 6 * (size_t)(zc + 6) * sizeof(double); }   // + z tables of one chunk
 };
 
@@ -574,9 +585,9 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   extern __shared__ unsigned char smem_raw[];
   unsigned char* base = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   double* planes = (double*)base;
-  double* X = (double*)(base + SM::NPL * SM::plane_stride);
-  double* Y = X + NF * XSTR;
-  uint64_t* mbar = (uint64_t*)(Y + NF * YSTR);
+  constexpr bool ONEBAR = SM::ONEBAR;
+  double* const XY0 = (double*)(base + SM::NPL * SM::plane_stride);   // parity buffer 0: X fields, then Y fields; buffer 1 follows (ONEBAR)
+  uint64_t* mbar = (uint64_t*)(XY0 + SM::NXY * SM::XYSTR);
   double* priv = (double*)(mbar + 8) + (threadIdx.x & (TY * TX - 1));   // private slots of the owner threads, field stride TY*TX
   double* gtab = (double*)(mbar + 8) + SM::NPRIV * TY * TX;   // spherical builds: column / row factor tables
   double* zt = gtab + SM::GT_N;   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
@@ -876,11 +887,17 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   auto march = [&](auto own_tag) {
   constexpr bool OWN = decltype(own_tag)::value;
   int bc = 1;                 // buffer of plane p
+  int xyo = 0;                // ONEBAR: offset of this plane's exchange buffer (toggles between the two parity buffers)
   for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
     const int pk = p + NG;
     const int bn = (bc == 2) ? 0 : bc + 1;
     double* Pc = planes + bc * PSTR;
     double* Pn = planes + bn * PSTR;
+    double* const X = XY0 + xyo;                          // exchange slots of this plane
+    double* const Y = X + NF * XSTR;
+    double* const Xo = XY0 + (ONEBAR ? SM::XYSTR - xyo : 0);   // ... and of the previous plane (fluxes through its upper x / y faces)
+    double* const Yo = Xo + NF * XSTR;
+    if (ONEBAR) xyo = SM::XYSTR - xyo;
     mbar_wait(&mbar[bn], (phase >> bn) & 1u);            // plane p+1 has arrived (issued a whole iteration ago)
     phase ^= (1u << bn);
 
@@ -992,6 +1009,25 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           zpn[2 + sv] = priv[(4 * (sv - 5) + 3) * PS];
         }
       }
+      // fluxes through the upper x and y faces of a cell come back in its own slots (written by the neighbours across
+      // those faces): into the partially updated cell Up
+      auto upper_xy = [&](const double* Xs, const double* Ys) {
+        struct { double p0, xp, p1, yp; } Kp;
+        Kp.p0 = GTAB ? GX(1) : k0p;
+        Kp.xp = GTAB ? GX(3) : kxp;
+        Kp.p1 = GTAB ? GX(4) * GY(1) : k1p;
+        Kp.yp = GTAB ? GX(4) * GY(3) : kyp;
+        if (EMON) {
+          EA -= fma(Kp.p0, Xs[NV * XSTR + xs_own], Kp.p1 * Ys[NV * YSTR + ys_own]);
+          DV += fma(Kp.p0, Xs[(NV + 1) * XSTR + xs_own], Kp.p1 * Ys[(NV + 1) * YSTR + ys_own]);
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? Kp.xp : Kp.p0), Xs[v * XSTR + xs_own], Up[v]);
+        if (SPH) Up[1] = fma(hgr, Ys[2 * YSTR + ys_own], Up[1]);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? Kp.yp : Kp.p1), Ys[v * YSTR + ys_own], Up[v]);
+      };
+      if (ONEBAR) upper_xy(Xo, Yo);                      // cell p-1: its neighbours wrote these during the previous plane, before barrier (1)
       double Fx[NV], Fy[NV], Fz[NV];
       double phx = 0.0, ufx = 0.0, phy = 0.0, ufy = 0.0, phz = 0.0, ufz = 0.0;
       {
@@ -1095,22 +1131,10 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Pn_p = Pn_c;
         }
       }
-      asm volatile("bar.sync 0;" ::: "memory");          // (2) fluxes visible
-      // ======== block 3: fluxes through the upper x and y faces come back in the own slots ================
-      struct { double p0, xp, p1, yp; } Kp;
-      Kp.p0 = GTAB ? GX(1) : k0p;
-      Kp.xp = GTAB ? GX(3) : kxp;
-      Kp.p1 = GTAB ? GX(4) * GY(1) : k1p;
-      Kp.yp = GTAB ? GX(4) * GY(3) : kyp;
-      if (EMON) {
-        EA -= fma(Kp.p0, X[NV * XSTR + xs_own], Kp.p1 * Y[NV * YSTR + ys_own]);
-        DV += fma(Kp.p0, X[(NV + 1) * XSTR + xs_own], Kp.p1 * Y[(NV + 1) * YSTR + ys_own]);
+      if (!ONEBAR) {
+        asm volatile("bar.sync 0;" ::: "memory");        // (2) fluxes visible
+        upper_xy(X, Y);                                  // block 3: fluxes through the upper x and y faces of cell p
       }
-#pragma unroll
-      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? Kp.xp : Kp.p0), X[v * XSTR + xs_own], Up[v]);
-      if (SPH) Up[1] = fma(hgr, Y[2 * YSTR + ys_own], Up[1]);
-#pragma unroll
-      for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? Kp.yp : Kp.p1), Y[v * YSTR + ys_own], Up[v]);
     } else {
       // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
       convert_plane(Pn, Wn);
@@ -1159,7 +1183,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           X[(NV + 1) * XSTR + xs_nbr] = uf;
         }
       }
-      asm volatile("bar.sync 0;" ::: "memory");          // (2)
+      if (!ONEBAR) asm volatile("bar.sync 0;" ::: "memory");   // (2)
     }
     bc = bn;
   }
