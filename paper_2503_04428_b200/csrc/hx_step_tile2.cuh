@@ -76,6 +76,9 @@ struct Args {
 // One CTA-wide barrier per plane instead of two: the exchange slots are double buffered by plane parity, so the flux a
 // neighbour writes back into a slot during plane p is picked up after the barrier of plane p+1 while the "+" states
 // of plane p+1 already sit in the other buffer.  Needs twice the slot memory: field counts whose buffers fit.
+#ifndef HX_T2_UNROLL
+#define HX_T2_UNROLL 1
+#endif
 #ifndef HX_T2_ONEBAR
 #define HX_T2_ONEBAR 1
 #endif
@@ -888,6 +891,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   constexpr bool OWN = decltype(own_tag)::value;
   int bc = 1;                 // buffer of plane p
   int xyo = 0;                // ONEBAR: offset of this plane's exchange buffer (toggles between the two parity buffers)
+  constexpr int UNR = HX_T2_UNROLL;
+#pragma unroll UNR
   for (int p = k0 - 1; p <= k1; ++p, outp += L.sz) {
     const int pk = p + NG;
     const int bn = (bc == 2) ? 0 : bc + 1;

@@ -30,7 +30,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t s
     if (e != cudaSuccess) return e;
     attr_set = smem;
   }
-  plan.name = EMON ? "tile2_emon" : (UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
+  plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
   kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();
 }
