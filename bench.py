@@ -47,18 +47,23 @@ WORKLOADS = {
     "sod_1d": (lambda: wl.sod_1d(1000), lambda: wl.sod_1d(1000)),
     # small case for quick checks of this script
     "rt_3d_small": (lambda: wl.rt_3d((128, 128, 128)), lambda: wl.rt_3d((48, 48, 48))),
+    "wedge_3d_small": (lambda: wl.wedge_3d((256, 64, 64)), lambda: wl.wedge_3d((96, 24, 24))),
 }
 DEFAULT_WORKLOAD = "rt_3d"
 
 
 def alg_flops_per_cell(spec):
-    """Algorithmic fp64 flops per 3-D cell-update (hand count from O1-O7 with every
-    predictor and face flux computed once; + and x count 1 each, so an FMA is 2; div and sqrt 1 each):
-    629 for nvar = 5, HLLC/HLL + minmod; +4 per slope for MC / van Leer, +6 van Albada; +84 per passive
-    scalar; +31 gravity; +65 spherical sources; +1025 for the gas + radiation EOS (Newton solves for T)."""
+    """Algorithmic fp64 flops per cell-update (hand count from O1-O7 with every predictor and
+    face flux computed once; + and x count 1 each, so an FMA is 2; div and sqrt 1 each).
+    3-D: 629 for nvar = 5, HLLC/HLL + minmod; +4 per slope for MC / van Leer, +6 van Albada; +84 per passive
+    scalar; +31 gravity; +65 spherical sources; +1025 for the gas + radiation EOS (Newton solves for T).
+    2-D (Cartesian): 380 for nvar = 4 (cons->prim 9, slopes 40, face states 32, cons + analytic flux of 4 face states
+    80, 4 predicted states 68, U^n 8, 2 HLLC 94, update 32, CFL rate 17); +50 per passive scalar; +20 gravity."""
     ns = spec["nvar"] - 2 - spec["ndim"]
     nvar = spec["nvar"]
     lim_extra = {wl.LIM_NONE: -1, wl.LIM_MINMOD: 0, wl.LIM_VANLEER: 4, wl.LIM_VANALBADA: 6, wl.LIM_MC: 4}[spec["limiter"]]
+    if spec["ndim"] == 2:
+        return 380 + 50 * ns + 2 * nvar * lim_extra + (20 if spec["gravity"] != wl.GRAV_NONE else 0)
     f = 629 + 84 * ns + 3 * nvar * lim_extra
     if spec["gravity"] != wl.GRAV_NONE:
         f += 31

@@ -44,7 +44,8 @@ enum { HX_CONSERVED = 0, HX_PRIMITIVE = 1 };
 /* Step kernel selection (hx_set_option(HX_OPT_KERNEL, ..)): AUTO picks the fused tile kernel where
  * it applies and the generic one elsewhere; the other two force one path (tests, profiling). */
 enum { HX_OPT_KERNEL = 0, HX_OPT_TIMING = 1 /* 0/1: bracket each step-kernel launch with CUDA events */ };
-enum { HX_KERNEL_AUTO = 0, HX_KERNEL_GENERIC = 1, HX_KERNEL_TILED = 2 /* the fused tile kernel ("tile2"), what AUTO picks in 3-D */ };
+enum { HX_KERNEL_AUTO = 0, HX_KERNEL_GENERIC = 1,
+       HX_KERNEL_TILED = 2 /* the fused TMA-staged tile kernels ("tile2*" in 3-D, "tile2d*" on 2-D Cartesian grids): what AUTO picks where they apply */ };
 
 #define HX_MAX_NVAR 16
 
@@ -103,7 +104,7 @@ long long hx_launch_count(const hx_handle* h);
  * measured so far, and their number.  Read after a synchronising call (hx_compute_dt / hx_get_state);
  * a launch whose events were not yet collected when the next step started is not counted. */
 int hx_kernel_time(hx_handle* h, double* total_ms, long long* launches);
-/* Name of the step kernel the last hx_step used ("generic", "tile2", "tile2_uni"). */
+/* Name of the step kernel the last hx_step used ("generic", "tile2", "tile2_uni", "tile2_rad", "tile2_emon", "tile2_emon_uni", "tile2d", "tile2d_uni"). */
 const char* hx_step_kernel_name(const hx_handle* h);
 const char* hx_last_error(const hx_handle* h);
 /* Device probe (no handle, default stream, synchronous): measured FP64 FMA throughput of the current

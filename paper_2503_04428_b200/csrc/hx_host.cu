@@ -248,8 +248,8 @@ int build_tables(hx_handle* h) {
   }
   // Bitwise-uniform Cartesian grid (e.g. 2^k cells on a dyadic extent): every cell of an axis has the same
   // hw, 1/width and 1/(centre distance), so the step kernel may take them as constants without changing a bit.
-  h->uniform = !sph && c.ndim == 3;
-  for (int d = 0; d < 3 && h->uniform; ++d) {
+  h->uniform = !sph && c.ndim >= 2;
+  for (int d = 0; d < c.ndim && h->uniform; ++d) {
     for (int p = 1; p < L.np[d]; ++p)
       if (memcmp(&pool[hw[d] + p], &pool[hw[d]], 8) || memcmp(&pool[iw[d] + p], &pool[iw[d]], 8) ||
           memcmp(&pool[idx[d] + p], &pool[idx[d] + 1], 8))

@@ -1,12 +1,36 @@
 // hx_step_tile2.cu -- host side of the fused 3-D step kernel (hx_step_tile2.cuh): tensor maps over the
 // padded SoA state, launch geometry, uniform-grid detection, dispatch on the field count.
 #include <cstring>
+#include <map>
+#include <mutex>
+#include <utility>
 
 #include "hx_step_tile2_launch.cuh"
 
 namespace hx {
 
 using t2::Plan;
+
+// 2-D kernel (hx_step_tile2d.cu)
+int tile2d_supported(const Layout& L, const Phys& P);
+cudaError_t tile2d_plan_fill(Plan* p, const Layout& L, double* const U[2], const double* uni, void* enc_fn);
+cudaError_t launch_step_tile2d(Plan* plan, const StepArgs& s, int cur, cudaStream_t st);
+
+cudaError_t t2::set_smem_limit(const void* kern, size_t smem) {
+  static std::mutex mu;
+  static std::map<std::pair<const void*, int>, size_t> done;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  size_t& have = done[std::make_pair(kern, dev)];
+  if (have < smem) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    have = smem;
+  }
+  return cudaSuccess;
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -37,6 +61,7 @@ static size_t smem_fixed(int nv) {   // shared memory of one CTA without the z t
 static bool nv_supported(int nv) { return nv == 5 || nv == 6 || nv == 7 || nv == 9; }
 
 int tile2_supported(const Layout& L, const Phys& P) {
+  if (L.ndim == 2) return tile2d_supported(L, P);
   if (P.emon_eps > 0.0 && !(L.nvar == 5 && !P.spherical && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MC && P.riemann == HX_RIEMANN_HLLC &&
                             P.eos == HX_EOS_IDEAL))
     return 0;   // internal-energy monitoring (Eq. 10-12): one tile instantiation (cold_stream_3d), else the generic kernel
@@ -51,6 +76,16 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], 
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   Plan* p = new Plan();
+  if (L.ndim == 2) {
+    cudaError_t e2 = tile2d_plan_fill(p, L, U, uni, (void*)enc);
+    if (e2 != cudaSuccess) {
+      delete p;
+      return e2;
+    }
+    *out = p;
+    return cudaSuccess;
+  }
+  p->ndim = 3;
   constexpr int TY = t2::TY_DEFAULT;
   const int ntx = (L.n[0] + t2::TX - 1) / t2::TX, nty = (L.n[1] + TY - 1) / TY;
   // z chunks: every chunk re-reads 4 planes and recomputes 2 predictor planes (+ a prologue), and with one CTA per
@@ -109,6 +144,7 @@ void tile2_plan_destroy(Plan* p) { delete p; }
 const char* tile2_kernel_name(const Plan* p) { return p ? p->name : "tile2"; }
 
 cudaError_t launch_step_tile2(Plan* plan, const StepArgs& s, int cur, cudaStream_t st) {
+  if (plan->ndim == 2) return launch_step_tile2d(plan, s, cur, st);
   t2::Args a;
   a.s = s;
   a.zc = plan->zc;

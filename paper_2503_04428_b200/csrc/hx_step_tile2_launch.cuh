@@ -8,7 +8,8 @@ namespace t2 {
 
 struct Plan {
   CUtensorMap tmap[2];
-  int zc;
+  int ndim;          // 3: hx_step_tile2.cuh (march along z); 2: hx_step_tile2d.cuh (march along y)
+  int zc;            // planes (rows in 2-D) per chunk of the march direction
   dim3 grid;
   bool uni;          // bitwise-uniform Cartesian tables: geometry travels as kernel-parameter constants
   bool grav_z;       // uniform gravity along direction 2 only
@@ -19,17 +20,17 @@ struct Plan {
 template <int NV>
 cudaError_t launch_nv(Plan& plan, const Args& a, int cur, cudaStream_t st);
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: raise it (never lower it) once per
+// (kernel, device), under a lock -- handles of one process may live on several GPUs and step from several threads.
+cudaError_t set_smem_limit(const void* kern, size_t smem);
+
 template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EOS_IDEAL, bool EMON = false>
 static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   constexpr int TY = TY_DEFAULT;
   auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY, EOS, EMON>;
   const size_t smem = Smem<NV, TY>::total(plan.zc);
-  static size_t attr_set = 0;
-  if (attr_set < smem) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = smem;
-  }
+  cudaError_t e = set_smem_limit((const void*)kern, smem);
+  if (e != cudaSuccess) return e;
   plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
   kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();

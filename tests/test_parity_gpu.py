@@ -444,6 +444,7 @@ def test_config_full_size_first_and_last_step(hx, oxlib, name):
     Ug, Uo = g.get_state(), o.get_state()
     l1 = l1_rel_per_field(Ug, Uo, ndim)
     assert max(l1) <= TOL_L1, (name, s, l1)
+    assert g.step_kernel == ("tile2d_uni" if name == "kh_2d" else "generic"), g.step_kernel
 
 
 def test_step_is_deterministic(hx):
