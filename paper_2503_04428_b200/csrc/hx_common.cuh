@@ -90,7 +90,9 @@ __device__ __forceinline__ double limited_slope(int lim, double a, double b) {
 // single-term roots the iterate can only move down towards the root; it stops when the correction is a few ulp.
 // ---------------------------------------------------------------------------------------------
 static __device__ __noinline__ double temperature_root(double a1, double a4, double b) {   // not inlined: keeps the generic kernels small (compile time)   // a1 T + a4 T^4 = b
-  if (!(b > 0.0)) return b / a1;                       // non-physical: a non-positive T makes the caller's P <= 0
+  // non-physical (e <= 0 or P <= 0): NaN, so that P, c_s and the CFL rate come out NaN and the callers' checks report it.
+  // (A negative T = b / a1 would NOT do: P = a_r T^4 / 3 + rho R T is positive again once a_r |T|^3 > 3 rho R.)
+  if (!(b > 0.0)) return __longlong_as_double(0x7ff8000000000000LL);
   double T = fmin(b / a1, sqrt(sqrt(b / a4)));
   for (int it = 0; it < 60; ++it) {                    // R27: until the correction is a few ulp; quadratic, ~5-9 steps
     const double T3 = T * T * T;

@@ -53,19 +53,23 @@ static size_t smem_fixed(int nv) {   // shared memory of one CTA without the z t
     case 5: return t2::Smem<5, TY>::fixed;
     case 6: return t2::Smem<6, TY>::fixed;
     case 7: return t2::Smem<7, TY>::fixed;
+    case 8: return t2::Smem<8, TY>::fixed;
     case 9: return t2::Smem<9, TY>::fixed;
+    case 10: return t2::Smem<10, TY>::fixed;
+    case 11: return t2::Smem<11, TY>::fixed;
     default: return 0;
   }
 }
 
-static bool nv_supported(int nv) { return nv == 5 || nv == 6 || nv == 7 || nv == 9; }
+// 3-D field counts with an instantiation: up to six passive scalars (nvar 11 is the largest whose planes, exchange
+// slots and private scalar slots fit into the 227 KB of shared memory a CTA can have)
+static bool nv_supported(int nv) { return nv >= 5 && nv <= 11; }
 
 int tile2_supported(const Layout& L, const Phys& P) {
   if (L.ndim == 2) return tile2d_supported(L, P);
   if (P.emon_eps > 0.0 && !(L.nvar == 5 && !P.spherical && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MC && P.riemann == HX_RIEMANN_HLLC &&
                             P.eos == HX_EOS_IDEAL))
     return 0;   // internal-energy monitoring (Eq. 10-12): one tile instantiation (cold_stream_3d), else the generic kernel
-  if (P.eos != HX_EOS_IDEAL && L.nvar != 9) return 0;   // gas + radiation EOS: tile kernel instantiated for nvar 9 only, else generic
   return L.ndim == 3 && nv_supported(L.nvar) && L.n[0] >= 2 && L.n[1] >= 2 && L.n[2] >= 2;
 }
 
@@ -158,7 +162,10 @@ cudaError_t launch_step_tile2(Plan* plan, const StepArgs& s, int cur, cudaStream
     case 5: return t2::launch_nv<5>(*plan, a, cur, st);
     case 6: return t2::launch_nv<6>(*plan, a, cur, st);
     case 7: return t2::launch_nv<7>(*plan, a, cur, st);
+    case 8: return t2::launch_nv<8>(*plan, a, cur, st);
     case 9: return t2::launch_nv<9>(*plan, a, cur, st);
+    case 10: return t2::launch_nv<10>(*plan, a, cur, st);
+    case 11: return t2::launch_nv<11>(*plan, a, cur, st);
     default: return cudaErrorNotSupported;
   }
 }

@@ -99,9 +99,9 @@ struct Smem {
   static constexpr int YSTR = (TY + 1) * TX;                   // y-exchange: slots ey = -1 .. TY-1
   static constexpr size_t x_bytes = (size_t)NF * XSTR * sizeof(double);
   static constexpr size_t y_bytes = (size_t)NF * YSTR * sizeof(double);
-  // nvar >= 9: the passive-scalar parts of the four predicted states an owner keeps across the first barrier go to
+  // nvar >= 8: the passive-scalar parts of the four predicted states an owner keeps across the first barrier go to
   // private shared-memory slots instead of registers (the nvar-9 builds spilled them to local memory: long-scoreboard stalls)
-  static constexpr int NPRIV = (NV >= 9) ? 4 * (NV - 5) : 0;
+  static constexpr int NPRIV = (NV >= 8) ? 4 * (NV - 5) : 0;
   static constexpr size_t priv_bytes = (size_t)NPRIV * TY * TX * sizeof(double);
   // spherical builds: 1-D factors of the update / CFL coefficients by tile column and tile row (7 + 7 tables), so that
   // their per-thread products need no registers (they used to be spilled: 20 doubles per thread)
@@ -221,7 +221,9 @@ __device__ __forceinline__ void tma_load_plane(const CUtensorMap* tmap, void* ds
 // Tg > 0: start from this guess instead (the temperature of the cell centre for its face and predicted states: a
 // start below the root overshoots once and then descends like any other; 2-3 steps instead of 6-8, same root).
 __device__ __forceinline__ double gr_temperature(double a1, double a4, double b, double Tg = 0.0) {
-  if (!(b > 0.0)) return b * rcp3(a1);                    // non-physical: T <= 0, hence P <= 0, which the rate check reports
+  // non-physical (e <= 0 or P <= 0): NaN -> P, c_s and the CFL rate are NaN and the rate check reports it (a negative T
+  // would give a POSITIVE radiation-dominated pressure a_r T^4 / 3 again)
+  if (!(b > 0.0)) return __longlong_as_double(0x7ff8000000000000LL);
   double T = (Tg > 0.0) ? Tg : dmin(b * rcp3(a1), sqrt3(sqrt3(b * rcp3(a4))));
   for (int it = 0; it < 60; ++it) {
     const double T3 = T * T * T;
@@ -802,7 +804,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       cs = sqrt3((P.gamma * P.gm1) * ir * e);
     } else {
       double pn;
-      gr_from_energy(P, Ul[0], ir, e, pn, cs);           // e <= 0 gives T <= 0 and a NaN sound speed, like the ideal branch
+      gr_from_energy(P, Ul[0], ir, e, pn, cs);           // e <= 0 gives T = NaN, hence a NaN sound speed, like the ideal branch
     }
     const double l0 = GTAB ? GX(5) : il0, l1 = GTAB ? GX(6) * GY(5) : il1, l2xy = GTAB ? GX(6) * GY(6) : il2xy;
     const double il2 = UNI ? a.uil[2] : l2xy * ZT(5, max(pkc, zb));

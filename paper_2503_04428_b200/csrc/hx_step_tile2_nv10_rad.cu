@@ -1,0 +1,13 @@
+// NV = 10 with the gas + radiation EOS (Eq. 6-7): spherical minmod + HLLC specialised build (the paper's supernova setup, L597: five scalars, point-mass gravity) and the two runtime-switch builds.  Own translation unit (compile time).
+#include "hx_step_tile2_launch.cuh"
+namespace hx {
+namespace t2 {
+cudaError_t launch_nv10_rad(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  const Phys& P = a.s.P;
+  if (P.spherical && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
+    return launch_cfg<10, true, GRAV_ANY, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
+  if (P.spherical) return launch_cfg<10, true, GRAV_ANY, -1, -1, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
+  return launch_cfg<10, false, GRAV_ANY, -1, -1, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
+}
+}  // namespace t2
+}  // namespace hx

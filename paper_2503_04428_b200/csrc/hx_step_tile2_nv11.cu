@@ -1,0 +1,12 @@
+// NV = 11 (3-D, six passive scalars): runtime-switch builds; the largest field count whose planes, exchange slots and private scalar slots fit into 227 KB of shared memory.
+#include "hx_step_tile2_launch.cuh"
+namespace hx {
+namespace t2 {
+cudaError_t launch_nv11_rad(Plan& plan, const Args& a, int cur, cudaStream_t st);
+template <>
+cudaError_t launch_nv<11>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv11_rad(plan, a, cur, st);
+  return launch_generic<11>(plan, a, cur, st);
+}
+}  // namespace t2
+}  // namespace hx

@@ -2,8 +2,10 @@
 #include "hx_step_tile2_launch.cuh"
 namespace hx {
 namespace t2 {
+cudaError_t launch_nv7_rad(Plan& plan, const Args& a, int cur, cudaStream_t st);
 template <>
 cudaError_t launch_nv<7>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv7_rad(plan, a, cur, st);   // Eq. 6-7: own translation unit
   const Phys& P = a.s.P;
   if (!P.spherical && plan.grav_z && P.limiter == HX_LIM_MC && P.riemann == HX_RIEMANN_HLLC) {
     if (plan.uni) return launch_cfg<7, false, GRAV_Z, HX_LIM_MC, HX_RIEMANN_HLLC, true>(plan, a, cur, st);

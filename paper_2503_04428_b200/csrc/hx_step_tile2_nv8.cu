@@ -1,0 +1,12 @@
+// NV = 8 (3-D, three passive scalars): runtime-switch builds.
+#include "hx_step_tile2_launch.cuh"
+namespace hx {
+namespace t2 {
+cudaError_t launch_nv8_rad(Plan& plan, const Args& a, int cur, cudaStream_t st);
+template <>
+cudaError_t launch_nv<8>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv8_rad(plan, a, cur, st);
+  return launch_generic<8>(plan, a, cur, st);
+}
+}  // namespace t2
+}  // namespace hx

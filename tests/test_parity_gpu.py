@@ -160,6 +160,46 @@ def test_every_bc_geometry_solver_limiter(hx, oxlib, case, kernel):
     assert max(rel) <= 3 * TOL_STEP, (case[0], rel)
 
 
+# field counts: every 3-D nvar from 5 to 11 (0..6 passive scalars; the paper's supernova runs carry five) runs
+# on the fused tile kernel, with the ideal gas and with the gas + radiation EOS; 2-D Cartesian nvar 4..8 on tile2d
+FIELD_CASES = [
+    # name, ndim, n, coords, bc_lo, bc_hi, gravity, limiter, riemann, ns
+    ("c3d_ns0", 3, [37, 11, 6], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 0),
+    ("c3d_ns3", 3, [37, 11, 6], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 3),
+    ("s3d_ns3", 3, [36, 10, 7], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 3),
+    ("c3d_ns5", 3, [37, 11, 6], 0, [2, 1, 2], [1, 2, 2], 1, 2, 0, 5),
+    ("s3d_ns5", 3, [36, 10, 7], 1, [2, 3, 3], [1, 3, 3], 2, 1, 1, 5),
+    ("s3d_ns5_hll_mc", 3, [36, 10, 7], 1, [2, 3, 3], [1, 3, 3], 2, 4, 0, 5),
+    ("c3d_ns6", 3, [37, 11, 6], 0, [0, 2, 1], [0, 2, 1], 0, 3, 1, 6),
+    ("s3d_ns6", 3, [36, 10, 7], 1, [2, 3, 0], [1, 3, 0], 3, 1, 1, 6),
+    ("c3d_ns0_rad", 3, [37, 11, 6], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 0),
+    ("s3d_ns1_rad", 3, [36, 10, 7], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 1),
+    ("c3d_ns3_rad", 3, [37, 11, 6], 0, [0, 2, 1], [0, 2, 1], 1, 2, 0, 3),
+    ("s3d_ns5_rad", 3, [36, 10, 7], 1, [2, 3, 3], [1, 3, 3], 2, 1, 1, 5),
+    ("s3d_ns6_rad", 3, [36, 10, 7], 1, [2, 3, 0], [1, 3, 0], 2, 4, 1, 6),
+    ("c2d_ns0", 2, [300, 9], 0, [2, 0], [1, 0], 1, 2, 1, 0),
+    ("c2d_ns2", 2, [261, 12], 0, [0, 1], [0, 2], 1, 4, 1, 2),
+    ("c2d_ns4_hll", 2, [70, 40], 0, [1, 2], [2, 1], 0, 1, 0, 4),
+    ("c2d_first_order", 2, [33, 7], 0, [0, 0], [0, 0], 0, 0, 1, 1),
+]
+
+
+@pytest.mark.parametrize("case", FIELD_CASES, ids=[c[0] for c in FIELD_CASES])
+def test_every_field_count_on_the_tile_kernels(hx, oxlib, case):
+    ox = oxlib
+    spec, W = random_problem(ox, case)
+    g, o = make_pair(hx, ox, spec, W, "auto")
+    for _ in range(3):
+        dt = 0.5 * o.compute_dt(0.5)
+        assert abs(0.5 * g.compute_dt(0.5) - dt) <= 1e-13 * dt
+        g.step(dt)
+        o.step(dt)
+    want = "tile2d" if spec["ndim"] == 2 else ("tile2_rad" if spec["eos"] else "tile2")
+    assert g.step_kernel == want, (case[0], g.step_kernel)
+    rel = max_rel_per_field(g.get_state(), o.get_state(), spec["ndim"])
+    assert max(rel) <= 3 * TOL_STEP, (case[0], rel)
+
+
 @pytest.mark.parametrize("lim", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("riemann", [0, 1])
 def test_limiters_and_solvers_3d(hx, oxlib, lim, riemann):
@@ -231,6 +271,37 @@ def test_nonphysical_state_is_reported_not_floored(hx):
         g.step(-1.0)
     # a far too large time step drives the update non-physical: reported at the next sync call
     g.step(50.0 * g.compute_dt(0.5))
+    with pytest.raises(hx.HxError) as e:
+        g.compute_dt(0.5)
+    assert e.value.code == hx.ERR_NONPHYSICAL
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_negative_internal_energy_is_reported_with_the_gas_radiation_eos(hx, kernel):
+    """Eq. 6-7, radiation dominated: e < 0 must be reported even though a naive T = e / a1 < 0 would give the positive
+    pressure a_r T^4 / 3 + rho R T again (rho = R = a_r = 1, gamma = 5/3, e = -10015: T = -6677, P ~ 6.6e14)."""
+    spec, W = wl.smooth_periodic(3, [40, 12, 10], seed=3, n_scalars=0)
+    spec = dict(spec, eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=1.0, gamma=5.0 / 3.0)
+    g = hx.Hydro(spec)
+    if kernel == "generic":
+        g.set_option(hx.OPT_KERNEL, hx.KERNEL_GENERIC)
+    W = W.copy()
+    W[0], W[1], W[2], W[3] = 1.0, 0.0, 0.0, 0.0
+    g.set_state(W, hx.PRIMITIVE)
+    U = g.get_state()
+    assert g.compute_dt(0.5) > 0
+    bad = U.copy()
+    bad[4, 4, 5, 17] = -10015.0          # total energy = internal energy (gas at rest) < 0
+    g.set_state(bad, hx.CONSERVED)
+    with pytest.raises(hx.HxError) as e:
+        g.compute_dt(0.5)                # stand-alone rate kernel
+    assert e.value.code == hx.ERR_NONPHYSICAL
+    # through the step kernel and its folded-in check: step from the bad state with a dt chosen before it went bad
+    g.set_state(U, hx.CONSERVED)
+    dt = g.compute_dt(0.5)
+    g.set_state(bad, hx.CONSERVED)
+    g.step(1e-3 * dt)
+    assert g.step_kernel == ("generic" if kernel == "generic" else "tile2_rad")
     with pytest.raises(hx.HxError) as e:
         g.compute_dt(0.5)
     assert e.value.code == hx.ERR_NONPHYSICAL
