@@ -75,7 +75,7 @@ int tile2_supported(const Layout& L, const Phys& P) {
 
 // uni: non-null when every per-axis table of this Cartesian grid is bitwise constant; then uni[0..2] = hw*idx and
 // uni[3..5] = 1/delta of the three axes.
-cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], const double* uni, int grav_z, Plan** out) {
+cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, Plan** out) {
   *out = nullptr;
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
@@ -123,6 +123,7 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys&, double* const U[2], 
   p->grid = dim3((unsigned)ntx, (unsigned)nty, (unsigned)nzc);
   p->uni = uni != nullptr;
   p->grav_z = grav_z != 0;
+  p->grav_r = P.spherical && (P.gravity == HX_GRAV_POINT_MASS || P.gravity == HX_GRAV_SELF);
   for (int d = 0; d < 3; ++d) {
     p->uf[d] = uni ? uni[d] : 0.0;
     p->uiw[d] = uni ? uni[3 + d] : 0.0;

@@ -47,22 +47,29 @@ constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows (two warpgroups) + 4 ring
 // Register budgets after setmaxnreg.  The pool is what the CTA was given at launch, (TY+4) warps x 32 x REGS_LAUNCH
 // (not the whole 64 K file): the owners' increase must fit into what the ring warpgroup releases, or
 // setmaxnreg.inc waits forever.
-// Measured (A/B on B200): ring 96..120 is equal for the Cartesian builds; the spherical ring path (nine fields,
-// geometric sources) spills below ~136 and then holds the owners up at the barriers (5.0 -> 6.6 Gcell/s).
+// Measured (A/B on B200): ring 96..120 is equal for the Cartesian builds.  The spherical ring path used to need 136
+// (nine fields at once, per-thread geometry products); with the scalars advanced one at a time (RING2) and the geometry
+// read from the shared column / row tables it runs in 120 like the Cartesian one from eight fields on (wedge_3d, nvar 9:
+// 104 -> 7.78 ms, 120 -> 7.31, 136 -> 7.51); the nvar 5-7 spherical builds keep 136 (sedov_wedge_3d: 1.14 vs 1.18 ms).
+#ifndef HX_T2_REGS_RING_SPH
+#define HX_T2_REGS_RING_SPH 120
+#endif
 #ifdef HX_T2_REGS_RING
-constexpr int ring_regs(bool) { return HX_T2_REGS_RING; }
+constexpr int ring_regs(bool, int) { return HX_T2_REGS_RING; }
 #else
-constexpr int ring_regs(bool sph) { return sph ? 136 : 120; }
+constexpr int ring_regs(bool sph, int nv) { return (sph && nv < 8) ? 136 : (sph ? HX_T2_REGS_RING_SPH : 120); }
 #endif
 constexpr int REGS_LAUNCH = (65536 / ((TY_DEFAULT + 4) * 32)) / 8 * 8;
-constexpr int owner_regs(bool sph) {
-  const int raw = (REGS_LAUNCH * (TY_DEFAULT + 4) - ring_regs(sph) * 4) / TY_DEFAULT / 8 * 8;
+constexpr int owner_regs(bool sph, int nv) {
+  const int raw = (REGS_LAUNCH * (TY_DEFAULT + 4) - ring_regs(sph, nv) * 4) / TY_DEFAULT / 8 * 8;
   return raw > 232 ? 232 : raw;
 }
-static_assert(owner_regs(true) * TY_DEFAULT + ring_regs(true) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
-static_assert(owner_regs(false) * TY_DEFAULT + ring_regs(false) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(true, 5) * TY_DEFAULT + ring_regs(true, 5) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(true, 9) * TY_DEFAULT + ring_regs(true, 9) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(false, 5) * TY_DEFAULT + ring_regs(false, 5) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
 
-enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2 };   // GRAV_Z: acceleration along direction 2 only
+enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2, GRAV_R = 3 };   // GRAV_Z / GRAV_R: acceleration along direction 2 / 0 only (uniform g along z; point mass, self-gravity)
+constexpr bool grav_has(int grav, int d) { return grav == GRAV_ANY || (grav == GRAV_Z && d == 2) || (grav == GRAV_R && d == 0); }
 
 struct Args {
   StepArgs s;
@@ -76,6 +83,9 @@ struct Args {
 // One CTA-wide barrier per plane instead of two: the exchange slots are double buffered by plane parity, so the flux a
 // neighbour writes back into a slot during plane p is picked up after the barrier of plane p+1 while the "+" states
 // of plane p+1 already sit in the other buffer.  Needs twice the slot memory: field counts whose buffers fit.
+#ifndef HX_T2_RING2_NV
+#define HX_T2_RING2_NV 8
+#endif
 #ifndef HX_T2_UNROLL
 #define HX_T2_UNROLL 1
 #endif
@@ -103,9 +113,10 @@ struct Smem {
   // private shared-memory slots instead of registers (the nvar-9 builds spilled them to local memory: long-scoreboard stalls)
   static constexpr int NPRIV = (NV >= 8) ? 4 * (NV - 5) : 0;
   static constexpr size_t priv_bytes = (size_t)NPRIV * TY * TX * sizeof(double);
-  // spherical builds: 1-D factors of the update / CFL coefficients by tile column and tile row (7 + 7 tables), so that
-  // their per-thread products need no registers (they used to be spilled: 20 doubles per thread)
-  static constexpr int GT_X = TX + 2, GT_Y = TY + 2, GT_N = 7 * (GT_X + GT_Y);
+  // spherical builds: 1-D factors of the slope, predictor, update and CFL coefficients by tile column and tile row
+  // (15 + 12 tables), read (and multiplied) at use, so that the ~27 loop-invariant per-thread products need no
+  // registers (they used to be spilled to local memory, which the 16 KB of L1 left beside the tile cannot hold)
+  static constexpr int GT_X = TX + 2, GT_Y = TY + 2, NGX = 15, NGY = 12, GT_N = NGX * GT_X + NGY * GT_Y;
   static constexpr int XYSTR = NF * (XSTR + YSTR);             // doubles of one parity buffer (X fields, then Y fields)
   static constexpr size_t fixed = NPL * plane_stride + NXY * (x_bytes + y_bytes) + priv_bytes + GT_N * sizeof(double) + 64 + 128;
   static constexpr size_t total(int zc) { return fixed + 6 * (size_t)(zc + 6) * sizeof(double); }   // + z tables of one chunk
@@ -584,13 +595,14 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   using SM = Smem<NV, TY>;
   constexpr int NF = SM::NF, FSTR = SM::FSTR, XSTR = SM::XSTR, YSTR = SM::YSTR, XP = SM::XP;
   constexpr int PSTR = (int)(SM::plane_stride / sizeof(double));
-  // column / row factor tables instead of per-thread products: measured +4 % on the spherical nvar-5 build, -2 % on
-  // the nvar-9 builds (their extra shared-memory loads sit on the critical path), hence only below nine fields
-  constexpr bool GTAB = SPH && NV < 9;
+  // column / row factor tables instead of per-thread products (spherical builds): frees ~50 registers per thread
+  constexpr bool GTAB = SPH;
+  constexpr bool GTABP = SPH && NV >= 8;   // ... also the slope / predictor coefficients: pays from eight fields on (below, -1.4 % on the nvar-5 wedge)
   extern __shared__ unsigned char smem_raw[];
   unsigned char* base = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   double* planes = (double*)base;
   constexpr bool ONEBAR = SM::ONEBAR;
+  constexpr bool RING2 = NV >= HX_T2_RING2_NV;   // ring warps: hydro fields first, then the passive scalars one at a time
   double* const XY0 = (double*)(base + SM::NPL * SM::plane_stride);   // parity buffer 0: X fields, then Y fields; buffer 1 follows (ONEBAR)
   uint64_t* mbar = (uint64_t*)(XY0 + SM::NXY * SM::XYSTR);
   double* priv = (double*)(mbar + 8) + (threadIdx.x & (TY * TX - 1));   // private slots of the owner threads, field stride TY*TX
@@ -679,8 +691,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     hcgt = hdt * crg * T.gt[pj];
     hcAt = hdt * crg * T.At[pj];
   }
-  const double hgx = (GRAV == GRAV_ANY) ? hdt * T.grav[0][pi] : 0.0;
-  const double hgy = (GRAV == GRAV_ANY) ? hdt * T.grav[1][pj] : 0.0;
+  const double hgx = grav_has(GRAV, 0) ? hdt * T.grav[0][pi] : 0.0;
+  const double hgy = grav_has(GRAV, 1) ? hdt * T.grav[1][pj] : 0.0;
 
   // ---- TMA prologue: planes k0-2, k0-1, k0 -------------------------------------------------------------
   const int xs = i0 + L.lead, ys = j0;                      // box origin in storage coordinates (cell i0-2, j0-2)
@@ -702,34 +714,65 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     zt[4 * zlen + q] = T.grav[2][pz];
     zt[5 * zlen + q] = T.lf[2][2][pz];
   }
-  if (GTAB) {   // 2 dt/2 dS/dV factors of the x and y faces by column (with the (1 -+ rr) of Eq. 14), by row (with (1 -+ st)), CFL lengths
+  if (GTAB) {   // column factors (with the (1 -+ rr) of Eq. 14) and row factors (with (1 -+ st)), (dt/2) folded in
     for (int e = threadIdx.x; e < SM::GT_X; e += blockDim.x) {
       const int pe = min(max(i0 + e - 1 + NG, 1), L.np[0] - 2);
-      const double km = 2.0 * hdt * T.cf[0][0][0][pe], kp = 2.0 * hdt * T.cf[0][1][0][pe], rr = T.rr[pe];
-      gtab[0 * SM::GT_X + e] = km;
-      gtab[1 * SM::GT_X + e] = kp;
-      gtab[2 * SM::GT_X + e] = km * (1.0 - rr);
-      gtab[3 * SM::GT_X + e] = kp * (1.0 + rr);
-      gtab[4 * SM::GT_X + e] = 2.0 * hdt * T.cr[pe];
-      gtab[5 * SM::GT_X + e] = T.lf[0][0][pe];
-      gtab[6 * SM::GT_X + e] = T.lf[1][0][pe];
+      const double km = 2.0 * hdt * T.cf[0][0][0][pe], kp = 2.0 * hdt * T.cf[0][1][0][pe], rr = T.rr[pe], hwx = T.hw[0][pe];
+      double* g = gtab + e;
+      g[0 * SM::GT_X] = km;
+      g[1 * SM::GT_X] = kp;
+      g[2 * SM::GT_X] = km * (1.0 - rr);
+      g[3 * SM::GT_X] = kp * (1.0 + rr);
+      g[4 * SM::GT_X] = 2.0 * hdt * T.cr[pe];
+      g[5 * SM::GT_X] = T.lf[0][0][pe];
+      g[6 * SM::GT_X] = T.lf[1][0][pe];
+      g[7 * SM::GT_X] = hwx * T.idx[0][pe];                 // flx
+      g[8 * SM::GT_X] = hwx * T.idx[0][pe + 1];             // fhx
+      g[9 * SM::GT_X] = hdt * T.cf[0][0][0][pe];            // hcm0
+      g[10 * SM::GT_X] = hdt * T.cf[0][1][0][pe];           // hcp0
+      g[11 * SM::GT_X] = hdt * T.cr[pe];                    // (dt/2) x the radial factor of the theta / phi face coefficients
+      g[12 * SM::GT_X] = hdt * T.gr[pe];                    // hgr
+      g[13 * SM::GT_X] = hdt * T.Ar[pe];                    // hAr
+      g[14 * SM::GT_X] = hdt * T.grav[0][pe];               // hgx
     }
-    double* gy = gtab + 7 * SM::GT_X;
+    double* gy = gtab + SM::NGX * SM::GT_X;
     for (int e = threadIdx.x; e < SM::GT_Y; e += blockDim.x) {
       const int pe = min(max(j0 + e - 1 + NG, 1), L.np[1] - 2);
-      const double bm = T.cf[1][0][1][pe], bp = T.cf[1][1][1][pe], st = T.st[pe];
-      gy[0 * SM::GT_Y + e] = bm;
-      gy[1 * SM::GT_Y + e] = bp;
-      gy[2 * SM::GT_Y + e] = bm * (1.0 - st);
-      gy[3 * SM::GT_Y + e] = bp * (1.0 + st);
-      gy[4 * SM::GT_Y + e] = T.cf[2][1][1][pe];
-      gy[5 * SM::GT_Y + e] = T.lf[1][1][pe];
-      gy[6 * SM::GT_Y + e] = T.lf[2][1][pe];
+      const double bm = T.cf[1][0][1][pe], bp = T.cf[1][1][1][pe], st = T.st[pe], hwy = T.hw[1][pe];
+      double* g = gy + e;
+      g[0 * SM::GT_Y] = bm;
+      g[1 * SM::GT_Y] = bp;
+      g[2 * SM::GT_Y] = bm * (1.0 - st);
+      g[3 * SM::GT_Y] = bp * (1.0 + st);
+      g[4 * SM::GT_Y] = T.cf[2][1][1][pe];
+      g[5 * SM::GT_Y] = T.lf[1][1][pe];
+      g[6 * SM::GT_Y] = T.lf[2][1][pe];
+      g[7 * SM::GT_Y] = hwy * T.idx[1][pe];                 // fly
+      g[8 * SM::GT_Y] = hwy * T.idx[1][pe + 1];             // fhy
+      g[9 * SM::GT_Y] = T.gt[pe];
+      g[10 * SM::GT_Y] = T.At[pe];
+      g[11 * SM::GT_Y] = hdt * T.grav[1][pe];               // hgy
     }
   }
   auto ZT = [&](int k, int pz) { return zt[k * zlen + (pz - zb)]; };
   auto GX = [&](int k) { return gtab[k * SM::GT_X + ex + 1]; };                       // column factor k of this thread's cell
-  auto GY = [&](int k) { return gtab[7 * SM::GT_X + k * SM::GT_Y + ey + 1]; };         // row factor k
+  auto GY = [&](int k) { return gtab[SM::NGX * SM::GT_X + k * SM::GT_Y + ey + 1]; };   // row factor k
+  // the loop-invariant coefficients of this thread's column: table reads at use (GTAB) or the registers set up above
+  auto FLX = [&]() { return GTABP ? GX(7) : flx; };
+  auto FHX = [&]() { return GTABP ? GX(8) : fhx; };
+  auto FLY = [&]() { return GTABP ? GY(7) : fly; };
+  auto FHY = [&]() { return GTABP ? GY(8) : fhy; };
+  auto HCM0 = [&]() { return GTABP ? GX(9) : hcm0; };
+  auto HCP0 = [&]() { return GTABP ? GX(10) : hcp0; };
+  auto HCM1 = [&]() { return GTABP ? GX(11) * GY(0) : hcm1; };
+  auto HCP1 = [&]() { return GTABP ? GX(11) * GY(1) : hcp1; };
+  auto C2M = [&]() { return GTABP ? GX(11) * GY(4) : c2m; };
+  auto HGR = [&]() { return GTABP ? GX(12) : hgr; };
+  auto HAR = [&]() { return GTABP ? GX(13) : hAr; };
+  auto HCGT = [&]() { return GTABP ? GX(11) * GY(9) : hcgt; };
+  auto HCAT = [&]() { return GTABP ? GX(11) * GY(10) : hcAt; };
+  auto HGX = [&]() { return GTABP ? GX(14) : hgx; };
+  auto HGY = [&]() { return GTABP ? GY(11) : hgy; };
   __syncthreads();
   if (threadIdx.x == 0) {
 #pragma unroll
@@ -829,8 +872,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       const double hwz = ZT(0, pk);
       flz = hwz * ZT(1, pk);
       fhz = hwz * ZT(1, pk + 1);
-      hcm2 = c2m * ZT(2, pk);
-      hcp2 = (SPH ? c2m : c2p) * ZT(3, pk);   // spherical: both z faces share the (r, theta) factors
+      hcm2 = C2M() * ZT(2, pk);
+      hcp2 = (SPH ? C2M() : c2p) * ZT(3, pk);   // spherical: both z faces share the (r, theta) factors
     }
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
@@ -845,17 +888,17 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
+      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLX(), FHX());
     }
-    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hcm0, Uxm, dU, unc6 ? unc6 + 0 : nullptr, Tc);
-    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hcp0, Uxp, dU, unc6 ? unc6 + 1 : nullptr, Tc);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -FLX() : -lim_scale<LIM>(), HCM0(), Uxm, dU, unc6 ? unc6 + 0 : nullptr, Tc);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? FLX() : lim_scale<LIM>(), -HCP0(), Uxp, dU, unc6 ? unc6 + 1 : nullptr, Tc);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], fly, fhy);
+      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLY(), FHY());
     }
-    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hcm1, Uym, dU, unc6 ? unc6 + 2 : nullptr, Tc);
-    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hcp1, Uyp, dU, unc6 ? unc6 + 3 : nullptr, Tc);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -FLY() : -lim_scale<LIM>(), HCM1(), Uym, dU, unc6 ? unc6 + 2 : nullptr, Tc);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? FLY() : lim_scale<LIM>(), -HCP1(), Uyp, dU, unc6 ? unc6 + 3 : nullptr, Tc);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double dp = Wn[v] - Wc[v];
@@ -868,16 +911,19 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
       const double ur = Wc[1], ut = Wc[2], up = Wc[3], pr = Wc[4];
-      dU[1] = fma(fma(mcy, ut, fma(mcz, up, 2.0 * pr)), hgr, dU[1]);
-      dU[2] += fma(mcz, up, pr) * hcgt - mcy * ur * hAr;
-      dU[3] -= mcz * fma(ur, hAr, ut * hcAt);
+      dU[1] = fma(fma(mcy, ut, fma(mcz, up, 2.0 * pr)), HGR(), dU[1]);
+      dU[2] += fma(mcz, up, pr) * HCGT() - mcy * ur * HAR();
+      dU[3] -= mcz * fma(ur, HAR(), ut * HCAT());
     }
-    if (GRAV == GRAV_ANY) {
-      dU[1] = fma(rho, hgx, dU[1]);
-      dU[2] = fma(rho, hgy, dU[2]);
-      dU[4] = fma(mcx, hgx, fma(mcy, hgy, dU[4]));
+    if (grav_has(GRAV, 0)) {
+      dU[1] = fma(rho, HGX(), dU[1]);
+      dU[4] = fma(mcx, HGX(), dU[4]);
     }
-    if (GRAV != GRAV_OFF) {
+    if (grav_has(GRAV, 1)) {
+      dU[2] = fma(rho, HGY(), dU[2]);
+      dU[4] = fma(mcy, HGY(), dU[4]);
+    }
+    if (grav_has(GRAV, 2)) {
       const double hgz = hdt * ZT(4, pk);
       dU[3] = fma(rho, hgz, dU[3]);
       dU[4] = fma(mcz, hgz, dU[4]);
@@ -960,13 +1006,13 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           flz = hwz * ZT(1, pk);
           fhz = hwz * ZT(1, pk + 1);
         }
-        const double scx = UNI ? flx : lim_scale<LIM>(), scy = UNI ? fly : lim_scale<LIM>(), scz = UNI ? flz : lim_scale<LIM>();
+        const double scx = UNI ? FLX() : lim_scale<LIM>(), scy = UNI ? FLY() : lim_scale<LIM>(), scz = UNI ? flz : lim_scale<LIM>();
 #pragma unroll
         for (int sv = 5; sv < NV; ++sv) {
           const double* Ps = Pc + sv * FSTR + cidx;
           const double fc = Ps[0];
-          const double tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, flx, fhx);
-          const double ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, fly, fhy);
+          const double tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, FLX(), FHX());
+          const double ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, FLY(), FHY());
           const double dp = Pn[sv * FSTR + cidx] - fc;
           const double tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
           dzm[sv] = dp;
@@ -1030,7 +1076,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         }
 #pragma unroll
         for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && (v == 2 || v == 3)) ? Kp.xp : Kp.p0), Xs[v * XSTR + xs_own], Up[v]);
-        if (SPH) Up[1] = fma(hgr, Ys[2 * YSTR + ys_own], Up[1]);
+        if (SPH) Up[1] = fma(HGR(), Ys[2 * YSTR + ys_own], Up[1]);
 #pragma unroll
         for (int v = 0; v < NV; ++v) Up[v] = fma(-((SPH && v == 3) ? Kp.yp : Kp.p1), Ys[v * YSTR + ys_own], Up[v]);
       };
@@ -1078,21 +1124,27 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll
         for (int v = 0; v < NV; ++v) Unew[v] = fma(-k2p, Fz[v], Up[v]);
         if (SPH) {   // upper phi-face half of F^phi_phi in S_r and S_theta (Eq. 16 as read in R10, R11)
-          Unew[1] = fma(hgr, Fz[3], Unew[1]);
-          Unew[2] = fma(hcgt, Fz[3], Unew[2]);
+          Unew[1] = fma(HGR(), Fz[3], Unew[1]);
+          Unew[2] = fma(HCGT(), Fz[3], Unew[2]);
         }
         if (GRAV != GRAV_OFF) {   // time-centred (R13)
-          const double hgzp = hdt * ZT(4, pk - 1);
           const double rs = Un0 + Unew[0];
-          if (GRAV == GRAV_ANY) {
-            const double m1 = fma(rs, hgx, Unew[1]), m2 = fma(rs, hgy, Unew[2]);
-            Unew[4] = fma(Unm[0] + m1, hgx, fma(Unm[1] + m2, hgy, Unew[4]));
+          if (grav_has(GRAV, 0)) {
+            const double m1 = fma(rs, HGX(), Unew[1]);
+            Unew[4] = fma(Unm[0] + m1, HGX(), Unew[4]);
             Unew[1] = m1;
+          }
+          if (grav_has(GRAV, 1)) {
+            const double m2 = fma(rs, HGY(), Unew[2]);
+            Unew[4] = fma(Unm[1] + m2, HGY(), Unew[4]);
             Unew[2] = m2;
           }
-          const double m3 = fma(rs, hgzp, Unew[3]);
-          Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
-          Unew[3] = m3;
+          if (grav_has(GRAV, 2)) {
+            const double hgzp = hdt * ZT(4, pk - 1);
+            const double m3 = fma(rs, hgzp, Unew[3]);
+            Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
+            Unew[3] = m3;
+          }
         }
         if (EMON) {   // Eq. 11-12 for cell p-1: e1 from the total energy, e2 from Eq. 10 (dt folded into the coefficients), E reset
           const double eaf = fma(-k2p, phz, EA), dvf = fma(k2p, ufz, DV);
@@ -1122,14 +1174,14 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Up[v] = fma((SPH && v == 3) ? K.ym : K.m1, Fy[v], u);
         }
         if (SPH) {
-          Up[1] = fma(hgr, Fz[3] + Fy[2], Up[1]);
-          Up[2] = fma(hcgt, Fz[3], Up[2]);
+          Up[1] = fma(HGR(), Fz[3] + Fy[2], Up[1]);
+          Up[2] = fma(HCGT(), Fz[3], Up[2]);
         }
         if (GRAV != GRAV_OFF) {
           Un0 = Un[0];
-          Unm[0] = Un[1];
-          Unm[1] = Un[2];
-          Unm[2] = Un[3];
+          if (grav_has(GRAV, 0)) Unm[0] = Un[1];
+          if (grav_has(GRAV, 1)) Unm[1] = Un[2];
+          if (grav_has(GRAV, 2)) Unm[2] = Un[3];
         }
         if (EMON) {
           EA = fma(k2m, phz, fma(K.m0, phx, K.m1 * phy));
@@ -1145,8 +1197,63 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     } else {
       // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
       convert_plane(Pn, Wn);
-      predictor(std::integral_constant<int, NV>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, nullptr, Tc, ec);
       double q[NF];
+      if constexpr (RING2) {
+        // many fields: like the owners, the five hydro fields first and then the passive scalars one at a time (same
+        // arithmetic as the owner path), so that the ring path stays within its small register budget
+        double unc[6], irs;
+        predictor(std::integral_constant<int, 5>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, unc, Tc, ec);
+        const int ks = (wid == TY) ? 3 : ((wid == TY + 1) ? 2 : ((wid == TY + 2) ? 1 : 0));   // the face whose predicted state this warp provides
+        {
+          double Usel[5];
+#pragma unroll
+          for (int v = 0; v < 5; ++v) Usel[v] = (ks & 2) ? ((ks & 1) ? Uf[3][v] : Uf[2][v]) : ((ks & 1) ? Uf[1][v] : Uf[0][v]);
+          const double* const us[1] = {Usel};
+          double* const qo[1] = {q};
+          double* const io[1] = {&irs};
+          pred_states<5, 1, EOS>(P, us, dU, qo, io, Tc);
+        }
+        double flz, fhz;
+        if (UNI) {
+          flz = fhz = a.uf[2];
+        } else {
+          const double hwz = ZT(0, pk);
+          flz = hwz * ZT(1, pk);
+          fhz = hwz * ZT(1, pk + 1);
+        }
+        const double scx = UNI ? FLX() : lim_scale<LIM>(), scy = UNI ? FLY() : lim_scale<LIM>(), scz = UNI ? flz : lim_scale<LIM>();
+#pragma unroll
+        for (int sv = 5; sv < NV; ++sv) {
+          const double* Ps = Pc + sv * FSTR + cidx;
+          const double fc = Ps[0];
+          const double tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, FLX(), FHX());
+          const double ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, FLY(), FHY());
+          const double dp = Pn[sv * FSTR + cidx] - fc;
+          const double tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
+          dzm[sv] = dp;
+          double rf[6];
+          rf[0] = Uf[0][0] * fma(-scx, tx, fc);
+          rf[1] = Uf[1][0] * fma(scx, tx, fc);
+          rf[2] = Uf[2][0] * fma(-scy, ty, fc);
+          rf[3] = Uf[3][0] * fma(scy, ty, fc);
+          rf[4] = Uf[4][0] * fma(-scz, tz, fc);
+          rf[5] = Uf[5][0] * fma(scz, tz, fc);
+          double dUs = 0.0;
+#pragma unroll
+          for (int k = 0; k < 6; ++k) dUs = fma(rf[k], unc[k], dUs);
+          if (lim_none) dUs = 0.0;
+          const double rsel = (ks & 2) ? ((ks & 1) ? rf[3] : rf[2]) : ((ks & 1) ? rf[1] : rf[0]);
+          q[2 + sv] = (rsel + dUs) * irs;
+        }
+        if (wid == TY) {
+#pragma unroll
+          for (int v = 0; v < NF; ++v) Y[v * YSTR + ys_own] = q[v];
+        } else if (wid == TY + 2 && act) {
+#pragma unroll
+          for (int v = 0; v < NF; ++v) X[v * XSTR + xs_own] = q[v];
+        }
+      } else {
+      predictor(std::integral_constant<int, NV>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, nullptr, Tc, ec);
       if (wid == TY) {
         pred_state<NV, EOS>(P, Uf[3], dU, q, Tc);
 #pragma unroll
@@ -1161,6 +1268,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         }
       } else {
         pred_state<NV, EOS>(P, Uf[0], dU, q, Tc);
+      }
       }
       asm volatile("bar.sync 0;" ::: "memory");          // (1)
       if (wid == TY + 1) {
@@ -1196,11 +1304,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   }
   };
   if (owner) {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(owner_regs(SPH)));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(owner_regs(SPH, NV)));
     march(std::true_type{});
     cfl_rate(k1 + 1 + NG - 2);                           // the last cell written (plane k1-1)
   } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ring_regs(SPH)));
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ring_regs(SPH, NV)));
     march(std::false_type{});
   }
 

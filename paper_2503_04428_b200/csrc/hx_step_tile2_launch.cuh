@@ -13,6 +13,7 @@ struct Plan {
   dim3 grid;
   bool uni;          // bitwise-uniform Cartesian tables: geometry travels as kernel-parameter constants
   bool grav_z;       // uniform gravity along direction 2 only
+  bool grav_r;       // spherical point mass / self-gravity: acceleration along direction 0 only
   double uf[3], uiw[3];
   const char* name;
 };

@@ -4,8 +4,8 @@ namespace hx {
 namespace t2 {
 cudaError_t launch_nv10_rad(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   const Phys& P = a.s.P;
-  if (P.spherical && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
-    return launch_cfg<10, true, GRAV_ANY, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
+  if (P.spherical && plan.grav_r && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
+    return launch_cfg<10, true, GRAV_R, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
   if (P.spherical) return launch_cfg<10, true, GRAV_ANY, -1, -1, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
   return launch_cfg<10, false, GRAV_ANY, -1, -1, false, HX_EOS_GAS_RADIATION>(plan, a, cur, st);
 }

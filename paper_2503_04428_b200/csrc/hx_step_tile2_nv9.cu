@@ -8,8 +8,8 @@ template <>
 cudaError_t launch_nv<9>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   const Phys& P = a.s.P;
   if (P.eos == HX_EOS_GAS_RADIATION) return launch_nv9_rad(plan, a, cur, st);   // Eq. 6-7: own translation unit (compile time)
-  if (P.spherical && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
-    return launch_cfg<9, true, GRAV_ANY, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);
+  if (P.spherical && plan.grav_r && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)
+    return launch_cfg<9, true, GRAV_R, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);
   return launch_generic<9>(plan, a, cur, st);
 }
 }  // namespace t2

@@ -59,6 +59,7 @@ cudaError_t tile2d_plan_fill(Plan* p, const Layout& L, double* const U[2], const
   p->ndim = 2;
   p->uni = uni != nullptr;
   p->grav_z = false;
+  p->grav_r = false;
   for (int d = 0; d < 3; ++d) {
     p->uf[d] = uni ? uni[d] : 0.0;
     p->uiw[d] = uni ? uni[3 + d] : 0.0;

@@ -160,22 +160,23 @@ def rt_3d(n=512, seed=1004):
     return spec, W
 
 
-def wedge_3d(n=(1024, 256, 256), seed=1005):
+def wedge_3d(n=(1024, 256, 256), seed=1005, n_scalars=4):
     """C5: spherical wedge, supernova-envelope-like (shape of PAPER.md Sect. 5.5): r in [1,100]
     log-spaced, theta in pi/2 +- 0.35, phi in +-0.35, gamma 4/3, rho ~ r^-2.5 with 1 % noise,
     hydrostatic P under point-mass gravity GM = 1, thermal bomb E = 10 in the first 4 radial
     cells (reading R24), 4 composition shells split at r = 3, 8, 25, reflecting r_min / theta /
-    phi walls, transmissive r_max (R18), minmod + HLLC, CFL 0.6, 50 steps."""
+    phi walls, transmissive r_max (R18), minmod + HLLC, CFL 0.6, 50 steps.  n_scalars = 5 adds a fifth shell
+    boundary at r = 60 (the field count of the paper's supernova runs)."""
     nr, nt, nph = n
     fr = log_faces(1.0, 100.0, nr)
     ft = uniform_faces(math.pi / 2 - 0.35, math.pi / 2 + 0.35, nt)
     fph = uniform_faces(-0.35, 0.35, nph)
     gamma = 4.0 / 3.0
     spec = _spec("wedge_3d", 3, [nr, nt, nph], [fr, ft, fph], [BC_REFLECTING, BC_WEDGE, BC_WEDGE],
-                 [BC_TRANSMISSIVE, BC_WEDGE, BC_WEDGE], gamma, LIM_MINMOD, coords=SPHERICAL, n_scalars=4,
+                 [BC_TRANSMISSIVE, BC_WEDGE, BC_WEDGE], gamma, LIM_MINMOD, coords=SPHERICAL, n_scalars=n_scalars,
                  gravity=GRAV_POINT_MASS, GM=1.0, cfl=0.6, steps=50, seed=seed)
     r = centres(fr)
-    W = np.zeros((9, nph, nt, nr))
+    W = np.zeros((5 + n_scalars, nph, nt, nr))
     W[0] = (r ** -2.5)[None, None, :] * (1.0 + 0.01 * noise(seed, (nph, nt, nr)))
     p = r ** -3.5 / 3.5
     nb = min(4, nr)
@@ -183,8 +184,8 @@ def wedge_3d(n=(1024, 256, 256), seed=1005):
     v4 = (fr[nb] ** 3 - fr[0] ** 3) / 3.0 * omega
     p[:nb] += (gamma - 1.0) * 10.0 / v4
     W[4] = p[None, None, :]
-    edges = [0.0, 3.0, 8.0, 25.0, np.inf]
-    for s in range(4):
+    edges = [0.0, 3.0, 8.0, 25.0, 60.0][:n_scalars] + [np.inf]
+    for s in range(n_scalars):
         W[5 + s] = ((r >= edges[s]) & (r < edges[s + 1])).astype(np.float64)[None, None, :]
     return spec, W
 
@@ -226,6 +227,14 @@ def wedge_3d_rad(n=(1024, 256, 256), seed=1005):
     envelope (gas dominated, both terms matter) and about 16 in the bomb (radiation dominated)."""
     spec, W = wedge_3d(n, seed)
     spec = dict(spec, name="wedge_3d_rad", gamma=5.0 / 3.0, eos=EOS_GAS_RADIATION, eos_R=1.0, eos_ar=30.0)
+    return spec, W
+
+
+def wedge_3d_sn(n=(1024, 256, 256), seed=1005):
+    """The setup of the paper's second weak-scaling run ("3-D spherical, gas + radiation EOS, 5 passive
+    scalars, point-mass gravity"): wedge_3d_rad with five composition shells (nvar 10)."""
+    spec, W = wedge_3d(n, seed, n_scalars=5)
+    spec = dict(spec, name="wedge_3d_sn", gamma=5.0 / 3.0, eos=EOS_GAS_RADIATION, eos_R=1.0, eos_ar=30.0)
     return spec, W
 
 
