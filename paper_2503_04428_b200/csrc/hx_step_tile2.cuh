@@ -245,13 +245,18 @@ __device__ __forceinline__ double gr_temperature(double a1, double a4, double b,
   return T;
 }
 // P and c_s from (rho, 1/rho, e); e from (rho, P)
-__device__ __forceinline__ void gr_from_energy(const Phys& P, double rho, double ir, double e, double& p, double& c, double Tg = 0.0) {
+__device__ __forceinline__ void gr_from_energy(const Phys& P, double rho, double ir, double e, double& p, double& c, double Tg = 0.0, double* Tout = nullptr) {
   const double T = gr_temperature(rho * P.rgas * P.igm1, P.arad, e, Tg);
+  if (Tout) *Tout = T;
   const double T3 = T * T * T;
   const double pg = rho * P.rgas * T;
   p = fma(P.arad * (1.0 / 3.0) * T3, T, pg);
   const double al = P.arad * (1.0 / 3.0) * T3 * ir * rcp3(P.rgas);   // P_r / P_g
   c = sqrt3(fma(al, fma(16.0, al, 20.0), P.gamma * P.igm1) * rcp3(fma(12.0, al, P.igm1)) * P.rgas * T);
+}
+__device__ __forceinline__ double gr_energy_of_T(const Phys& P, double rho, double T) {   // Eq. 6a
+  const double T2 = T * T;
+  return fma(P.arad, T2 * T2, rho * P.rgas * T * P.igm1);
 }
 __device__ __forceinline__ double gr_energy(const Phys& P, double rho, double p, double Tg = 0.0, double* Tout = nullptr) {
   const double T = gr_temperature(rho * P.rgas, P.arad * (1.0 / 3.0), p, Tg);
@@ -260,11 +265,19 @@ __device__ __forceinline__ double gr_energy(const Phys& P, double rho, double p,
   return fma(P.arad, T2 * T2, rho * P.rgas * T * P.igm1);
 }
 
+template <int N>
+__device__ __forceinline__ void gr_from_energy_n(const Phys& P, const double* rho, const double* ir, const double* e, double* p, double* c, double Tg,
+                                                 double* Tout = nullptr);
+template <int N>
+__device__ __forceinline__ void gr_energy_n(const Phys& P, const double* rho, const double* p, double Tg, double* e);
+
 // ------------------------------------------------------------------------------------------------
 // Pointwise pieces of the scheme.  Field order of W / U: rho, u|m [3], P|E, scalars f|rho f.
 // ------------------------------------------------------------------------------------------------
+// gas + radiation EOS: coll = all 32 lanes of the warp are here together (the fast solve is warp-collective); Tg = a nearby
+// temperature to start it from; Tout: the temperature found
 template <int NV, int EOS = HX_EOS_IDEAL>
-__device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, double* W) {   // Eq. 1, Eq. 5 / 6
+__device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, double* W, bool coll = false, double Tg = 0.0, double* Tout = nullptr) {   // Eq. 1, Eq. 5 / 6
   const double ir = rcp3(U[0]);
   W[0] = U[0];
   W[1] = U[1] * ir;
@@ -275,7 +288,9 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
     W[4] = P.gm1 * fma(-0.5, ke2, U[4]);
   } else {
     double c;
-    gr_from_energy(P, U[0], ir, fma(-0.5, ke2, U[4]), W[4], c);
+    const double e = fma(-0.5, ke2, U[4]);
+    if (coll) gr_from_energy_n<1>(P, &U[0], &ir, &e, &W[4], &c, Tg, Tout);   // warp-collective: coll must be warp-uniform
+    else gr_from_energy(P, U[0], ir, e, W[4], c, 0.0, Tout);
   }
 #pragma unroll
   for (int s = 5; s < NV; ++s) W[s] = U[s] * ir;
@@ -286,7 +301,9 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
 // area/volume coefficient `coef` (Eq. 18: + for the lower face, - for the upper face).
 template <int NV, int DIR, int EOS = HX_EOS_IDEAL>
 __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, const double* t, double sc, double coef, double* Uf, double* dU,
-                                               double* unc_out = nullptr, double Tg = 0.0) {
+                                               double* unc_out = nullptr, double* pf_out = nullptr) {
+  // gas + radiation EOS: the internal energy e(rho_f, P_f) of the face state is left out here (Uf[4] and the energy flux);
+  // the caller solves for the six of a cell at once and adds them (pf_out: the face pressure it needs for that)
   double Wf[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) Wf[v] = fma(sc, t[v], Wc[v]);
@@ -296,7 +313,8 @@ __device__ __forceinline__ void face_cons_flux(const Phys& P, const double* Wc, 
   Uf[2] = r * Wf[2];
   Uf[3] = r * Wf[3];
   const double ke2 = fma(Uf[3], Wf[3], fma(Uf[2], Wf[2], Uf[1] * Wf[1]));
-  Uf[4] = fma(0.5, ke2, EOS == HX_EOS_IDEAL ? Wf[4] * P.igm1 : gr_energy(P, r, Wf[4], Tg));
+  Uf[4] = (EOS == HX_EOS_IDEAL) ? fma(0.5, ke2, Wf[4] * P.igm1) : 0.5 * ke2;
+  if (EOS != HX_EOS_IDEAL && pf_out) *pf_out = Wf[4];
   const double unc = Wf[1 + DIR] * coef;
   if (unc_out) *unc_out = unc;   // signed (dt/2) dS/dV u_n of this face: what a passive scalar's flux rides on
   dU[0] = fma(r, unc, dU[0]);
@@ -430,6 +448,84 @@ __device__ __forceinline__ void sqrt3_n(const double* x, double* y) {
   for (int k = 0; k < N; ++k) y[k] = fma(t[k], e[k], t[k]);
 }
 
+// N roots of a1 T + a4 T^4 = b at once, from the guess Tg > 0 (the temperature of a neighbouring state: the cell centre for
+// its face and predicted states, the cell below for a cell centre, the old time level for the new state).  Halley steps
+// (cubic convergence, f'' = 12 a4 T^2) advanced stage by stage for all N so that their dependent chains interleave, until
+// every instance in the warp has a correction below 2e-6 T -- the iterate after it is then converged to ~1e-17 (relative
+// error e -> 1.25 e^3) -- at most four; an instance that is not there yet (a strong shock, a non-physical input) goes
+// through the Newton loop.  f is increasing and convex for T > 0: the root is unique, so this is the oracle's root to
+// rounding (R27).  WARP-COLLECTIVE (the early exit is a warp vote): all 32 lanes must call it together, whatever their data;
+// a lane whose guess is not positive (first plane, garbage beyond the domain edge) takes the Newton loop afterwards.
+template <int N>
+__device__ __forceinline__ void gr_temperature_n(const double* a1, double a4, const double* b, double Tg, double* T) {
+  double t[N], s[N];
+  const bool guess = Tg > 0.0;                          // per lane; a lane without a usable guess idles through the collective part
+#pragma unroll
+  for (int k = 0; k < N; ++k) t[k] = guess ? Tg : 1.0;
+  const double a46 = 6.0 * a4;
+#pragma unroll 1
+  for (int it = 0; it < 4; ++it) {
+    double T2[N], q[N], f[N], fp[N], den[N], r[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) T2[k] = t[k] * t[k];
+#pragma unroll
+    for (int k = 0; k < N; ++k) q[k] = a4 * T2[k] * t[k];
+#pragma unroll
+    for (int k = 0; k < N; ++k) f[k] = fma(q[k], t[k], fma(a1[k], t[k], -b[k]));
+#pragma unroll
+    for (int k = 0; k < N; ++k) fp[k] = fma(4.0, q[k], a1[k]);
+#pragma unroll
+    for (int k = 0; k < N; ++k) den[k] = fma(fp[k], fp[k], -(f[k] * (a46 * T2[k])));
+    rcp3_n<N>(den, r);
+#pragma unroll
+    for (int k = 0; k < N; ++k) s[k] = f[k] * fp[k] * r[k];
+#pragma unroll
+    for (int k = 0; k < N; ++k) t[k] -= s[k];
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < N; ++k) ok = ok && (fabs(s[k]) <= 2e-6 * t[k]);
+    if (__all_sync(0xffffffffu, ok || !guess)) break;
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    T[k] = t[k];
+    if (!(guess && (b[k] > 0.0) && (fabs(s[k]) <= 2e-6 * t[k]))) T[k] = gr_temperature(a1[k], a4, b[k], (guess && t[k] > 0.0) ? t[k] : 0.0);
+  }
+}
+
+// P and c_s of N states from (rho, 1/rho, e) (Eq. 6b, Eq. 7); e of N states from (rho, P) (Eq. 6a)
+template <int N>
+__device__ __forceinline__ void gr_from_energy_n(const Phys& P, const double* rho, const double* ir, const double* e, double* p, double* c, double Tg,
+                                                 double* Tout) {
+  double a1[N], T[N], pr3[N], al[N], x[N], y[N], w[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) a1[k] = rho[k] * P.rgas * P.igm1;
+  gr_temperature_n<N>(a1, P.arad, e, Tg, T);
+  const double ar3 = P.arad * (1.0 / 3.0), irg = rcp3(P.rgas);
+#pragma unroll
+  for (int k = 0; k < N; ++k) pr3[k] = ar3 * (T[k] * T[k] * T[k]);
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    p[k] = fma(pr3[k], T[k], rho[k] * P.rgas * T[k]);
+    al[k] = pr3[k] * ir[k] * irg;                                   // P_r / P_g
+    x[k] = fma(12.0, al[k], P.igm1);
+    if (Tout) Tout[k] = T[k];
+  }
+  rcp3_n<N>(x, w);
+#pragma unroll
+  for (int k = 0; k < N; ++k) y[k] = fma(al[k], fma(16.0, al[k], 20.0), P.gamma * P.igm1) * w[k] * P.rgas * T[k];
+  sqrt3_n<N>(y, c);
+}
+template <int N>
+__device__ __forceinline__ void gr_energy_n(const Phys& P, const double* rho, const double* p, double Tg, double* e) {
+  double a1[N], T[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) a1[k] = rho[k] * P.rgas;
+  gr_temperature_n<N>(a1, P.arad * (1.0 / 3.0), p, Tg, T);
+#pragma unroll
+  for (int k = 0; k < N; ++k) e[k] = gr_energy_of_T(P, rho[k], T[k]);
+}
+
 // N predicted face states at once (same arithmetic as pred_state)
 template <int NV, int N, int EOS = HX_EOS_IDEAL>
 __device__ __forceinline__ void pred_states(const Phys& P, const double* const* Uf, const double* dU, double* const* q, double* const* ir_out = nullptr, double Tg = 0.0) {
@@ -459,8 +555,7 @@ __device__ __forceinline__ void pred_states(const Phys& P, const double* const* 
 #pragma unroll
     for (int k = 0; k < N; ++k) pr[k] = P.gm1 * e[k];
   } else {
-#pragma unroll
-    for (int k = 0; k < N; ++k) gr_from_energy(P, r[k], ir[k], e[k], pr[k], c[k], Tg);
+    gr_from_energy_n<N>(P, r, ir, e, pr, c, Tg);
   }
 #pragma unroll
   for (int k = 0; k < N; ++k) {
@@ -783,19 +878,21 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   }
 
   // raw conserved -> primitive of the cell at offset `off` of plane `pl`, in place if `store`
-  auto convert = [&](double* pl, int off, double* Wout, bool store) {
+  // (gas + radiation EOS: Tg > 0 = a nearby temperature to start the solve from -- warp-collective, so only where all 32
+  // lanes arrive together; Tout = the temperature found)
+  auto convert = [&](double* pl, int off, double* Wout, bool store, bool coll = false, double Tg = 0.0, double* Tout = nullptr) {
     double U[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) U[v] = pl[v * FSTR + off];
-    prim_of_cons<NV, EOS>(P, U, Wout);
+    prim_of_cons<NV, EOS>(P, U, Wout, coll, Tg, Tout);
     if (store) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) pl[v * FSTR + off] = Wout[v];
     }
   };
   // own cell + the ghost cells this thread is responsible for (every needed cell of the box exactly once)
-  auto convert_plane = [&](double* pl, double* Wown) {
-    convert(pl, cidx, Wown, act);
+  auto convert_plane = [&](double* pl, double* Wown, bool coll = false, double Tg = 0.0, double* Tout = nullptr) {
+    convert(pl, cidx, Wown, act, coll, Tg, Tout);
     if (xoff != 0 && act) {
       double tmp[NV];
       convert(pl, cidx + xoff, tmp, true);
@@ -804,13 +901,14 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   };
 
   double dzm[NV];             // W(p) - W(p-1) of this column
+  double Tcar = 0.0, Tprev = 0.0, Tul = 0.0;   // gas + radiation EOS: T^n of the own cell of plane p, of plane p-1, of the cell in Ul
   {
     double Wm2[NV], Wc0[NV];
     mbar_wait(&mbar[0], 0u);
     convert(planes, cidx, Wm2, false);
     mbar_wait(&mbar[1], 0u);
     phase = 3u;
-    convert_plane(planes + PSTR, Wc0);
+    convert_plane(planes + PSTR, Wc0, false, 0.0, &Tcar);
 #pragma unroll
     for (int v = 0; v < NV; ++v) dzm[v] = Wc0[v] - Wm2[v];
     __syncthreads();          // everyone has read plane k0-2: its buffer takes plane k0+1
@@ -847,7 +945,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       cs = sqrt3((P.gamma * P.gm1) * ir * e);
     } else {
       double pn;
-      gr_from_energy(P, Ul[0], ir, e, pn, cs);           // e <= 0 gives T = NaN, hence a NaN sound speed, like the ideal branch
+      gr_from_energy_n<1>(P, &Ul[0], &ir, &e, &pn, &cs, Tul);   // warp-collective; e <= 0 gives T = NaN, hence a NaN sound speed, like the ideal branch
     }
     const double l0 = GTAB ? GX(5) : il0, l1 = GTAB ? GX(6) * GY(5) : il1, l2xy = GTAB ? GX(6) * GY(6) : il2xy;
     const double il2 = UNI ? a.uil[2] : l2xy * ZT(5, max(pkc, zb));
@@ -883,30 +981,49 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // gas + radiation EOS: temperature and internal energy of the cell centre, the Newton start of its twelve face solves
     Tc = 0.0;
     ec = 0.0;
-    if (EOS != HX_EOS_IDEAL) ec = gr_energy(P, Wc[0], Wc[4], 0.0, &Tc);
+    if (EOS != HX_EOS_IDEAL) {   // T of the cell centre was found when its plane was converted; e from Eq. 6a
+      Tc = Tcar;
+      ec = gr_energy_of_T(P, Wc[0], Tc);
+    }
     double t[NVP];
+    double uncl[6], pfl[6];     // gas + radiation EOS: per face (dt/2) dS/dV u_n and the face pressure
+    double* const ul = unc6 ? unc6 : uncl;
+    constexpr bool GR = EOS != HX_EOS_IDEAL;
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLX(), FHX());
     }
-    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -FLX() : -lim_scale<LIM>(), HCM0(), Uxm, dU, unc6 ? unc6 + 0 : nullptr, Tc);
-    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? FLX() : lim_scale<LIM>(), -HCP0(), Uxp, dU, unc6 ? unc6 + 1 : nullptr, Tc);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -FLX() : -lim_scale<LIM>(), HCM0(), Uxm, dU, (unc6 || GR) ? ul + 0 : nullptr, pfl + 0);
+    face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? FLX() : lim_scale<LIM>(), -HCP0(), Uxp, dU, (unc6 || GR) ? ul + 1 : nullptr, pfl + 1);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
       t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLY(), FHY());
     }
-    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -FLY() : -lim_scale<LIM>(), HCM1(), Uym, dU, unc6 ? unc6 + 2 : nullptr, Tc);
-    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? FLY() : lim_scale<LIM>(), -HCP1(), Uyp, dU, unc6 ? unc6 + 3 : nullptr, Tc);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -FLY() : -lim_scale<LIM>(), HCM1(), Uym, dU, (unc6 || GR) ? ul + 2 : nullptr, pfl + 2);
+    face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? FLY() : lim_scale<LIM>(), -HCP1(), Uyp, dU, (unc6 || GR) ? ul + 3 : nullptr, pfl + 3);
 #pragma unroll
     for (int v = 0; v < NVP; ++v) {
       const double dp = Wn[v] - Wc[v];
       t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
       dzm[v] = dp;
     }
-    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, unc6 ? unc6 + 4 : nullptr, Tc);
-    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, unc6 ? unc6 + 5 : nullptr, Tc);
+    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, (unc6 || GR) ? ul + 4 : nullptr, pfl + 4);
+    face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, (unc6 || GR) ? ul + 5 : nullptr, pfl + 5);
+    if (GR) {   // internal energies of the six face states (P -> T -> e, Eq. 6), all at once, into E and the energy flux
+      const double rf[6] = {Uxm[0], Uxp[0], Uym[0], Uyp[0], Uzm[0], Uzp[0]};
+      double ef[6];
+      gr_energy_n<6>(P, rf, pfl, Tc, ef);
+      Uxm[4] += ef[0];
+      Uxp[4] += ef[1];
+      Uym[4] += ef[2];
+      Uyp[4] += ef[3];
+      Uzm[4] += ef[4];
+      Uzp[4] += ef[5];
+#pragma unroll
+      for (int k = 0; k < 6; ++k) dU[4] = fma(ef[k], ul[k], dU[4]);
+    }
     const double rho = Wc[0];
     const double mcx = rho * Wc[1], mcy = rho * Wc[2], mcz = rho * Wc[3];
     if (SPH) {   // cell-centred geometric sources (R8)
@@ -956,13 +1073,13 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 
     // Edge iterations (p = k0-1 and p = k1) run the same code on valid but unused data; only the global
     // store and the CFL rate are predicated, so the iteration is three straight-line blocks.
-    double Wn[NV], Wc[NV], dU[NV], hcm2, Tc, ec;
+    double Wn[NV], Wc[NV], dU[NV], hcm2, Tc, ec, Tn = 0.0;
     double Uf[6][NV];          // conserved face states: 0 x-, 1 x+, 2 y-, 3 y+, 4 z-, 5 z+
     if constexpr (OWN) {
       // ======== block 1: slopes, half-step increment, the six predicted states in two interleaved
       // batches, the deferred CFL rate of cell p-2 =============================================================
       cfl_rate(pk - 2);
-      convert(Pn, cidx, Wn, true);                       // [A] cons -> prim of the own cell of plane p+1, in place
+      convert(Pn, cidx, Wn, true, true, Tcar, &Tn);            // [A] cons -> prim of the own cell of plane p+1, in place (T started from the cell below)
       double unc[6], ir6[6];   // per face: signed (dt/2) dS/dV u_n of the face state, 1/rho of the predicted state
       predictor(std::integral_constant<int, 5>{}, Pc, Wn, pk, Wc, dU, Uf[0], Uf[1], Uf[2], Uf[3], Uf[4], Uf[5], hcm2, unc, Tc, ec);
       double qxm[NF], qym[NF], qzm[NF], zpn[NF];
@@ -1159,6 +1276,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         }
 #pragma unroll
         for (int v = 0; v < 5; ++v) Ul[v] = Unew[v];
+        if (EOS != HX_EOS_IDEAL) Tul = Tprev;              // T^n of cell p-1: where the solve for its new temperature starts
       }
       {   // cell p: U^n + the three lower faces
         const double k2m = 2.0 * hcm2;
@@ -1196,7 +1314,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       }
     } else {
       // ======== ring warps: predictor, one predicted state, at most one Riemann solve =====================
-      convert_plane(Pn, Wn);
+      convert_plane(Pn, Wn, true, Tcar, &Tn);
       double q[NF];
       if constexpr (RING2) {
         // many fields: like the owners, the five hydro fields first and then the passive scalars one at a time (same
@@ -1301,6 +1419,10 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       if (!ONEBAR) asm volatile("bar.sync 0;" ::: "memory");   // (2)
     }
     bc = bn;
+    if (EOS != HX_EOS_IDEAL) {
+      Tprev = Tcar;
+      Tcar = Tn;
+    }
   }
   };
   if (owner) {
