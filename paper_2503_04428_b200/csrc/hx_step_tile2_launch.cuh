@@ -38,11 +38,15 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t s
 }
 
 // the runtime-switch build (limiter, solver, any gravity) covers every configuration of this NV
-template <int NV>
+template <int NV, bool EMON = false>
 static cudaError_t launch_generic(Plan& plan, const Args& a, int cur, cudaStream_t st) {
-  if (a.s.P.spherical) return launch_cfg<NV, true, GRAV_ANY, -1, -1, false>(plan, a, cur, st);
-  return launch_cfg<NV, false, GRAV_ANY, -1, -1, false>(plan, a, cur, st);
+  if (a.s.P.spherical) return launch_cfg<NV, true, GRAV_ANY, -1, -1, false, HX_EOS_IDEAL, EMON>(plan, a, cur, st);
+  return launch_cfg<NV, false, GRAV_ANY, -1, -1, false, HX_EOS_IDEAL, EMON>(plan, a, cur, st);
 }
+
+// internal-energy monitoring (Eq. 10-12), ideal gas: one translation unit per NV (hx_step_tile2_nv<N>_emon.cu)
+template <int NV>
+cudaError_t launch_emon(Plan& plan, const Args& a, int cur, cudaStream_t st);
 
 }  // namespace t2
 }  // namespace hx

@@ -5,6 +5,7 @@ namespace t2 {
 cudaError_t launch_nv11_rad(Plan& plan, const Args& a, int cur, cudaStream_t st);
 template <>
 cudaError_t launch_nv<11>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.emon_eps > 0.0) return launch_emon<11>(plan, a, cur, st);   // Eq. 10-12 (ideal gas; checked by tile2_supported): own translation unit
   if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv11_rad(plan, a, cur, st);
   return launch_generic<11>(plan, a, cur, st);
 }

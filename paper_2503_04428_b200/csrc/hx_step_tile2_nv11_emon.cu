@@ -1,0 +1,10 @@
+// NV = 11 with the monitoring of the internal energy (Eq. 10-12): the two runtime-switch builds.
+#include "hx_step_tile2_launch.cuh"
+namespace hx {
+namespace t2 {
+template <>
+cudaError_t launch_emon<11>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  return launch_generic<11, true>(plan, a, cur, st);
+}
+}  // namespace t2
+}  // namespace hx

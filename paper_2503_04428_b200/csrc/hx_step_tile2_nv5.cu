@@ -6,12 +6,9 @@ namespace t2 {
 cudaError_t launch_nv5_rad(Plan& plan, const Args& a, int cur, cudaStream_t st);
 template <>
 cudaError_t launch_nv<5>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.emon_eps > 0.0) return launch_emon<5>(plan, a, cur, st);   // Eq. 10-12 (ideal gas; checked by tile2_supported): own translation unit
   if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv5_rad(plan, a, cur, st);   // Eq. 6-7: own translation unit
   const Phys& P = a.s.P;
-  if (P.emon_eps > 0.0) {   // internal-energy monitoring (Eq. 10-12): Cartesian, no gravity, MC + HLLC (cold_stream_3d); checked by tile2_supported
-    if (plan.uni) return launch_cfg<5, false, GRAV_OFF, HX_LIM_MC, HX_RIEMANN_HLLC, true, HX_EOS_IDEAL, true>(plan, a, cur, st);
-    return launch_cfg<5, false, GRAV_OFF, HX_LIM_MC, HX_RIEMANN_HLLC, false, HX_EOS_IDEAL, true>(plan, a, cur, st);
-  }
   if (!P.spherical && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC) {
     if (plan.uni) return launch_cfg<5, false, GRAV_OFF, HX_LIM_MINMOD, HX_RIEMANN_HLLC, true>(plan, a, cur, st);
     return launch_cfg<5, false, GRAV_OFF, HX_LIM_MINMOD, HX_RIEMANN_HLLC, false>(plan, a, cur, st);

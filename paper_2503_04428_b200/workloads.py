@@ -238,6 +238,27 @@ def wedge_3d_sn(n=(1024, 256, 256), seed=1005):
     return spec, W
 
 
+def wedge_3d_emon(n=(1024, 256, 256), seed=1007):
+    """SURVEY 8(f) rank 2 in the geometry the paper uses it for ("highly supersonic" supernova ejecta):
+    the C5 wedge (same grid, density, pressure without the bomb, four composition shells, point-mass gravity) as a cold
+    radial outflow u_r = 500 (Mach 800 at r = 1, 8000 at r = 100) with seeded velocity noise of 0.3 c_s in all three
+    components (subsonic in the comoving frame), transmissive radial faces, monitoring with the paper's epsilon = 1e-6.
+    e / e_k = 6.8e-6 / r: alpha = 1 inside r ~ 7, the blended branch of Eq. 12 out to r ~ 68, alpha = 0 (internal energy
+    from Eq. 10 alone) beyond.  (A homologous outflow u_r ~ r at this Mach number breaks the scheme in its first step
+    with or without monitoring: the Hancock predictor forms its pressures from the total energy, R29.)"""
+    spec, W = wedge_3d(n, seed)
+    nr, nt, nph = n
+    spec = dict(spec, name="wedge_3d_emon", emon_eps=1e-6)
+    spec["bc_lo"] = [BC_TRANSMISSIVE, BC_WEDGE, BC_WEDGE]
+    r = centres(spec["faces"][0])
+    W[4] = (r ** -3.5 / 3.5)[None, None, :] + 0.0 * W[4]          # no bomb
+    cs = np.sqrt(4.0 / 3.0 * (r ** -3.5 / 3.5) / r ** -2.5)
+    W[1] = 500.0 + 0.3 * cs[None, None, :] * noise(seed + 1, (nph, nt, nr))
+    W[2] = 0.3 * cs[None, None, :] * noise(seed + 2, (nph, nt, nr))
+    W[3] = 0.3 * cs[None, None, :] * noise(seed + 3, (nph, nt, nr))
+    return spec, W
+
+
 def wedge_3d_selfgrav(n=(1024, 256, 256), seed=1005):
     """the C5 wedge with the self-gravity of its envelope (Eq. 4) on top of the
     central mass: G M_c = 1 as in wedge_3d, G = 0.004, so that the spherically averaged envelope (mass 8 pi (sqrt(r) - 1)
