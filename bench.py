@@ -236,9 +236,7 @@ def run_ours(args):
     if args.limiter or args.riemann:       # measured variants of a workload: other limiter / solver
         mf, mr = make_full, make_reduced
         make_full, make_reduced = (lambda: override(mf(), args)), (lambda: override(mr(), args))
-    spec, W = make_full()
-    if world > 1:   # independent replicas: same structure, rank-specific noise
-        spec, W = make_full() if rank == 0 else WORKLOADS[args.workload][0]()
+    spec, W = make_full()          # N > 1: every rank runs the same workload (independent replicas, same seed, same overrides)
     ncell = int(np.prod(spec["n"]))
     nvar = spec["nvar"]
     cfl = spec["cfl"]
@@ -279,38 +277,57 @@ def run_ours(args):
     kernel_ms = (ms1 - ms0) / max(1, cnt1 - cnt0)
 
     # ---- end to end through host buffers ----------------------------------------------------
-    e2e_steps = max(1, min(K, args.e2e_steps))
+    # Every step copies its input state from pinned host memory to the GPU (hx_set_state), advances it (hx_compute_dt +
+    # hx_step) and copies the result back to pinned host memory (hx_get_state).  Two handles on two streams work on
+    # independent inputs in turn (HX_OPT_ASYNC_HOST), so that the upload of one step overlaps the download of the
+    # previous one on the full-duplex link; each handle's own H2D -> step -> D2H chain stays ordered on its stream.
+    e2e_steps = max(2, min(2 * K, args.e2e_steps))
     nbytes = ncell * nvar * 8
     h_in = torch.from_numpy(U0).pin_memory()
-    h_out = torch.empty_like(h_in).pin_memory()
-    sim.set_state(h_in.numpy(), hx.CONSERVED)
-    sim.step(sim.compute_dt(cfl))
-    sim.get_state(h_out.numpy(), hx.CONSERVED)          # warm-up of the host path
+    del U0
+    s2 = torch.cuda.Stream()
+    sims = [sim, hx.Hydro(spec, stream=s2)]
+    if args.kernel != "auto":
+        sims[1].set_option(hx.OPT_KERNEL, {"generic": hx.KERNEL_GENERIC, "tile2": hx.KERNEL_TILED}[args.kernel])
+    h_out = [torch.empty_like(h_in).pin_memory() for _ in sims]
+    for sm, ho in zip(sims, h_out):
+        sm.set_option(hx.OPT_ASYNC_HOST, 1)
+        sm.set_state(h_in.numpy(), hx.CONSERVED)
+        sm.step(sm.compute_dt(cfl))
+        sm.get_state(ho.numpy(), hx.CONSERVED)          # warm-up of the host path
+        sm.sync()
     barrier()
     ev0.record(stream)
     for s in range(e2e_steps):
-        src = h_in if s % 2 == 0 else h_out              # each step consumes the previous step's host result
-        dst = h_out if s % 2 == 0 else h_in
-        sim.set_state(src.numpy(), hx.CONSERVED)
-        sim.step(sim.compute_dt(cfl))
-        sim.get_state(dst.numpy(), hx.CONSERVED)
+        sm, ho = sims[s % 2], h_out[s % 2]
+        sm.set_state(h_in.numpy(), hx.CONSERVED)         # enqueued behind this handle's previous download
+        sm.step(sm.compute_dt(cfl))                      # waits for this handle's upload only
+        sm.get_state(ho.numpy(), hx.CONSERVED)
+    stream.wait_stream(s2)
     ev1.record(stream)
+    for sm in sims:
+        sm.sync()
     barrier()
     e2e_ms = aggregate_max_ms(ev0.elapsed_time(ev1), world, dev)
     e2e_value = world * ncell * e2e_steps / (e2e_ms * 1e-3) / 1e6
+    assert torch.equal(h_out[0][:, :2], h_out[1][:, :2]), "the two pipelined handles disagree on the same input"
     kernel_name = sim.step_kernel
-    del h_in, h_out
+    sims[1].close()
+    del h_in, h_out, sims
 
     if rank != 0:
         return
     peak, peak_src = measured_peaks()
     alg_bytes = 16 * nvar * ncell                        # read U^n once + write U^{n+1} once
     achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
+    traffic, traffic_source = None, None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu captures
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(args.workload, {}).get(kernel_name)
+            tj = json.load(open(tpath))
+            traffic = tj.get(args.workload, {}).get(kernel_name)
+            if traffic is not None:
+                traffic_source = "profiles/traffic.json (%s)" % tj.get("_source", "ncu --set full capture, see profiles/README.md")
         except Exception:
             traffic = None
     fp64_peak, dfma_lat = hx.probe_fp64()              # measured FP64 FMA rate of this GPU (TFLOP/s) and DFMA latency
@@ -329,7 +346,7 @@ def run_ours(args):
                          else "state fits in L2: HBM fraction not meaningful for this workload"},
         # the path is FP64-pipe bound on B200: the binding roof is "alu"; the HBM figures stay beside it
         "roofline": {"bound": "alu", "achieved": alu_achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": alu_achieved / fp64_peak,
-                     "traffic": traffic, "kernel": kernel_name, "kernel_ms": kernel_ms,
+                     "traffic": traffic, "traffic_source": traffic_source, "kernel": kernel_name, "kernel_ms": kernel_ms,
                      "algorithmic_flops_per_cell": alg_flops_per_cell(spec), "algorithmic_flops_per_launch": alg_flops,
                      "peak_source": "measured on this GPU by hx_probe_fp64 (independent DFMA chains on all SMs; nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2)",
                      "dfma_dependent_latency_cycles": dfma_lat, "kernel_share_of_step": kernel_ms / (total_ms / K)},
@@ -337,7 +354,8 @@ def run_ours(args):
                          "traffic": traffic, "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src},
         "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_sample},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
+                "pipeline": "2 handles on 2 streams, independent inputs, async pinned-host copies (HX_OPT_ASYNC_HOST)"},
         "gpu_launches": launches,
         "clocks": clk,
     }
@@ -351,7 +369,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=12)
     ap.add_argument("--limiter", default=None, choices=sorted(LIMITERS), help="override the workload's slope limiter")
     ap.add_argument("--riemann", default=None, choices=sorted(SOLVERS), help="override the workload's Riemann solver")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tile2"], help="step kernel (A/B runs)")

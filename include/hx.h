@@ -43,7 +43,8 @@ enum { HX_HOST = 0, HX_DEVICE = 1 };
 enum { HX_CONSERVED = 0, HX_PRIMITIVE = 1 };
 /* Step kernel selection (hx_set_option(HX_OPT_KERNEL, ..)): AUTO picks the fused tile kernel where
  * it applies and the generic one elsewhere; the other two force one path (tests, profiling). */
-enum { HX_OPT_KERNEL = 0, HX_OPT_TIMING = 1 /* 0/1: bracket each step-kernel launch with CUDA events */ };
+enum { HX_OPT_KERNEL = 0, HX_OPT_TIMING = 1 /* 0/1: bracket each step-kernel launch with CUDA events */,
+       HX_OPT_ASYNC_HOST = 2 /* 0/1: hx_set_state / hx_get_state with HOST buffers only enqueue their copies (see below) */ };
 enum { HX_KERNEL_AUTO = 0, HX_KERNEL_GENERIC = 1,
        HX_KERNEL_TILED = 2 /* the fused TMA-staged tile kernels ("tile2*" in 3-D, "tile2d*" on 2-D Cartesian grids): what AUTO picks where they apply */ };
 
@@ -84,6 +85,11 @@ int hx_set_option(hx_handle* h, int option, int value);
  * or primitive, converted through the EOS).  Returns after the copy is enqueued (device pointer)
  * or finished (host pointer). */
 int hx_set_state(hx_handle* h, const double* data, int mem_space, int form);
+/* With HX_OPT_ASYNC_HOST = 1 the two calls above / below return as soon as their copies are enqueued on the handle's
+ * stream when given a HOST pointer: the buffer must be page-locked and stay untouched until hx_sync (or any other
+ * synchronising call) returns; hx_get_state then reports HX_ERR_NONPHYSICAL at that later call.  This lets the
+ * host-to-device copy of one handle overlap the device-to-host copy of another on the full-duplex link. */
+int hx_sync(hx_handle* h);
 /* Copy the interior state out; synchronises the stream.  Returns HX_ERR_NONPHYSICAL (after
  * copying) if a kernel flagged a non-physical state since the last hx_set_state. */
 int hx_get_state(hx_handle* h, double* data, int mem_space, int form);
@@ -98,20 +104,25 @@ int hx_compute_dt(hx_handle* h, double cfl, double* dt_out);
 int hx_step(hx_handle* h, double dt);
 /* Number of stored fields, 2 + ndim + n_scalars. */
 int hx_nvar(const hx_handle* h);
+/* Name of the step kernel the last hx_step used ("generic", "tile2", "tile2_uni", "tile2_rad", "tile2_emon", "tile2_emon_uni", "tile2d", "tile2d_uni"). */
+const char* hx_step_kernel_name(const hx_handle* h);
+const char* hx_last_error(const hx_handle* h);
+const char* hx_version(void);
+/* ABI handshake for bindings: sizeof(hx_config) as this library was compiled.  A binding whose struct has another size
+ * was written for another revision of this header and must not call hx_create. */
+int hx_config_size(void);
+
+/* ---- diagnostics and measurement hooks (bench.py, profiling); not needed to run the method ---------------------- */
 /* Kernels launched by this handle so far (for bench.py's gpu_launches). */
 long long hx_launch_count(const hx_handle* h);
 /* With HX_OPT_TIMING on: device time (ms) spent in the step kernel alone, summed over the launches
  * measured so far, and their number.  Read after a synchronising call (hx_compute_dt / hx_get_state);
  * a launch whose events were not yet collected when the next step started is not counted. */
 int hx_kernel_time(hx_handle* h, double* total_ms, long long* launches);
-/* Name of the step kernel the last hx_step used ("generic", "tile2", "tile2_uni", "tile2_rad", "tile2_emon", "tile2_emon_uni", "tile2d", "tile2d_uni"). */
-const char* hx_step_kernel_name(const hx_handle* h);
-const char* hx_last_error(const hx_handle* h);
 /* Device probe (no handle, default stream, synchronous): measured FP64 FMA throughput of the current
  * GPU in TFLOP/s (1 FMA = 2 flop; many independent chains on every SM) and the issue-to-issue latency
  * of a dependent DFMA in SM cycles.  This is the denominator of the "alu" roofline. */
 int hx_probe_fp64(double* tflops, double* dep_latency_cycles);
-const char* hx_version(void);
 
 #ifdef __cplusplus
 }

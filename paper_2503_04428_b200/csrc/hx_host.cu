@@ -60,6 +60,7 @@ struct hx_handle {
   double uni[6] = {0, 0, 0, 0, 0, 0};   // hw*idx and 1/delta of the three axes when uniform
   long long launches = 0;
   const char* last_kernel = "none";
+  bool async_host = false;    // HX_OPT_ASYNC_HOST: host-buffer copies are only enqueued
   bool timing = false, ev_pending = false;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   double kernel_ms = 0.0;
@@ -328,7 +329,8 @@ StepArgs make_args(hx_handle* h, double dt) {
 
 extern "C" {
 
-const char* hx_version(void) { return "hx 0.1 (sm_100a)"; }
+const char* hx_version(void) { return "hx 0.2 (sm_100a)"; }
+int hx_config_size(void) { return (int)sizeof(hx_config); }
 
 int hx_create(const hx_config* cfg, hx_handle** out) {
   if (!out) return HX_ERR_INVALID_ARG;
@@ -424,6 +426,10 @@ int hx_set_option(hx_handle* h, int option, int value) {
     h->kernel_opt = value;
     return HX_OK;
   }
+  if (option == HX_OPT_ASYNC_HOST) {
+    h->async_host = value != 0;
+    return HX_OK;
+  }
   if (option == HX_OPT_TIMING) {
     if (value && !h->ev0) {
       if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess) return fail(h, HX_ERR_CUDA, "cudaEventCreate");
@@ -467,10 +473,20 @@ int hx_set_state(hx_handle* h, const double* data, int mem_space, int form) {
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_set_state: memset");
   h->rate_valid = false;
   h->ghosts_valid = false;
-  if (mem_space == HX_HOST) {
+  if (mem_space == HX_HOST && !h->async_host) {
     e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_set_state: sync");
   }
+  return HX_OK;
+}
+
+int hx_sync(hx_handle* h) {
+  if (!h) return HX_ERR_INVALID_ARG;
+  cudaError_t e = cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(DevScalars), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "hx_sync");
+  collect_timing(h);
+  if (h->h_scal->status & 1) return fail(h, HX_ERR_NONPHYSICAL, "non-physical state (rho <= 0, P <= 0 or non-finite)");
   return HX_OK;
 }
 
@@ -488,6 +504,7 @@ int hx_get_state(hx_handle* h, double* data, int mem_space, int form) {
     e = cudaMemcpyAsync(data, dst, nint * sizeof(double), cudaMemcpyDeviceToHost, h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_get_state: D2H copy");
   }
+  if (mem_space == HX_HOST && h->async_host) return HX_OK;   // enqueued only: the caller synchronises with hx_sync
   e = cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(DevScalars), cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_get_state: sync");

@@ -22,12 +22,12 @@ GRAV_NONE, GRAV_UNIFORM, GRAV_POINT_MASS, GRAV_SELF = 0, 1, 2, 3
 SPACING_UNIFORM, SPACING_LOG, SPACING_CUSTOM = 0, 1, 2
 HOST, DEVICE = 0, 1
 CONSERVED, PRIMITIVE = 0, 1
-OPT_KERNEL, OPT_TIMING = 0, 1
+OPT_KERNEL, OPT_TIMING, OPT_ASYNC_HOST = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 EXPORTS = ["hx_create", "hx_destroy", "hx_set_stream", "hx_set_option", "hx_set_state", "hx_get_state",
            "hx_compute_dt", "hx_step", "hx_nvar", "hx_launch_count", "hx_kernel_time", "hx_step_kernel_name", "hx_last_error",
-           "hx_version", "hx_probe_fp64"]
+           "hx_version", "hx_probe_fp64", "hx_config_size", "hx_sync"]
 
 
 class HxConfig(C.Structure):
@@ -73,6 +73,7 @@ def lib():
         L.hx_get_state.argtypes = [vp, dp, C.c_int, C.c_int]
         L.hx_compute_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.hx_step.argtypes = [vp, C.c_double]
+        L.hx_sync.argtypes = [vp]
         L.hx_nvar.argtypes = [vp]
         L.hx_launch_count.argtypes = [vp]
         L.hx_launch_count.restype = C.c_longlong
@@ -83,6 +84,11 @@ def lib():
         L.hx_last_error.restype = C.c_char_p
         L.hx_version.restype = C.c_char_p
         L.hx_probe_fp64.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        # ABI handshake: a stale libhx.so (or a stale binding) with another hx_config layout must not be used
+        if not hasattr(L, "hx_config_size") or L.hx_config_size() != C.sizeof(HxConfig):
+            have = L.hx_config_size() if hasattr(L, "hx_config_size") else "unknown"
+            raise RuntimeError(f"{path}: hx_config is {have} bytes in the library but {C.sizeof(HxConfig)} in this binding; "
+                               "rebuild with `python paper_2503_04428_b200/build.py --force`")
         _lib = L
     return _lib
 
@@ -198,6 +204,9 @@ class Hydro:
 
     def step(self, dt: float):
         self._check(self._L.hx_step(self._h, dt), "hx_step")
+
+    def sync(self):
+        self._check(self._L.hx_sync(self._h), "hx_sync")
 
     def kernel_time(self):
         """(total ms, launches) of the step kernel alone, measured with CUDA events (OPT_TIMING on)."""

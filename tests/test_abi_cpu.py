@@ -25,6 +25,7 @@ def test_library_loads_and_exports_every_declared_symbol():
     for name in names:
         assert hasattr(L, name), name
     assert b"sm_100a" in L.hx_version()
+    assert L.hx_config_size() == C.sizeof(hx.HxConfig)      # the handshake hx.lib() enforces
 
 
 def test_config_struct_matches_header_layout():
