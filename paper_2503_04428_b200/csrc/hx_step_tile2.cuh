@@ -290,7 +290,7 @@ __device__ __forceinline__ void prim_of_cons(const Phys& P, const double* U, dou
     double c;
     const double e = fma(-0.5, ke2, U[4]);
     if (coll) gr_from_energy_n<1>(P, &U[0], &ir, &e, &W[4], &c, Tg, Tout);   // warp-collective: coll must be warp-uniform
-    else gr_from_energy(P, U[0], ir, e, W[4], c, 0.0, Tout);
+    else gr_from_energy(P, U[0], ir, e, W[4], c, Tg, Tout);   // Newton loop, from the guess when it is positive
   }
 #pragma unroll
   for (int s = 5; s < NV; ++s) W[s] = U[s] * ir;
@@ -895,8 +895,8 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     convert(pl, cidx, Wown, act, coll, Tg, Tout);
     if (xoff != 0 && act) {
       double tmp[NV];
-      convert(pl, cidx + xoff, tmp, true);
-      if (coff != 0) convert(pl, cidx + coff, tmp, true);
+      convert(pl, cidx + xoff, tmp, true, false, Tg);   // lane-divergent: the per-lane Newton loop, started from the neighbour's T
+      if (coff != 0) convert(pl, cidx + coff, tmp, true, false, Tg);
     }
   };
 
