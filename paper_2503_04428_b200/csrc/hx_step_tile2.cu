@@ -67,6 +67,7 @@ static bool nv_supported(int nv) { return nv >= 5 && nv <= 11; }
 
 int tile2_supported(const Layout& L, const Phys& P) {
   if (L.ndim == 2) return tile2d_supported(L, P);
+  if (P.spherical && P.gravity == HX_GRAV_UNIFORM) return 0;   // a constant (r, theta, phi) acceleration vector: generic kernel (the spherical tile builds carry no phi gravity)
   if (P.emon_eps > 0.0 && P.eos != HX_EOS_IDEAL) return 0;   // internal-energy monitoring (Eq. 10-12) with the gas + radiation EOS: generic kernel
   return L.ndim == 3 && nv_supported(L.nvar) && L.n[0] >= 2 && L.n[1] >= 2 && L.n[2] >= 2;
 }
@@ -102,13 +103,15 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2]
   }
   const long long cols = (long long)ntx * nty;
   // the chunk's z tables live in shared memory next to the plane ring and the exchange buffers (227 KB per CTA)
-  const size_t fixed = smem_fixed(L.nvar);
-  const size_t budget = 227 * 1024 - 1024;   // static shared memory of the block reduction + reserve
+  constexpr int TYs = t2::TY_DEFAULT;
+  const size_t fixed = smem_fixed(L.nvar) + (P.spherical ? (size_t)t2::Smem<5, TYs>::GT_N * 8 : 0);   // (GT_N does not depend on the field count)
+  const size_t var_per_plane = (size_t)t2::Smem<5, TYs>::nzt(P.spherical != 0) * 8;
+  const size_t budget = 227 * 1024 - 256;    // 256 B of static shared memory: the block reduction of the CFL rate
   int nzc = (L.n[2] + 15) / 16;
   double best = -1.0;
   for (int c = 1; c <= (L.n[2] + 15) / 16; ++c) {
     const int zc = (L.n[2] + c - 1) / c, chunks = (L.n[2] + zc - 1) / zc;
-    if (fixed + 6 * (size_t)(zc + 6) * 8 > budget) continue;
+    if (fixed + var_per_plane * (size_t)(zc + 6) > budget) continue;
     const double waves = (double)(cols * chunks) / sms;
     const double eff = (double)L.n[2] / ((double)chunks * (zc + 3)) * waves / (double)(long long)(waves + 0.999999);
     if (eff > best + 1e-9) {

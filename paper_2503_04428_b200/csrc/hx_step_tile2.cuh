@@ -69,7 +69,9 @@ static_assert(owner_regs(true, 9) * TY_DEFAULT + ring_regs(true, 9) * 4 <= REGS_
 static_assert(owner_regs(false, 5) * TY_DEFAULT + ring_regs(false, 5) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
 
 enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2, GRAV_R = 3 };   // GRAV_Z / GRAV_R: acceleration along direction 2 / 0 only (uniform g along z; point mass, self-gravity)
-constexpr bool grav_has(int grav, int d) { return grav == GRAV_ANY || (grav == GRAV_Z && d == 2) || (grav == GRAV_R && d == 0); }
+constexpr bool grav_has(int grav, int d, bool sph = false) {
+  return (grav == GRAV_ANY && !(sph && d == 2)) || (grav == GRAV_Z && d == 2) || (grav == GRAV_R && d == 0);   // spherical builds: never along phi
+}
 
 struct Args {
   StepArgs s;
@@ -92,7 +94,10 @@ struct Args {
 #ifndef HX_T2_ONEBAR
 #define HX_T2_ONEBAR 1
 #endif
-constexpr bool one_barrier(int nv) { return HX_T2_ONEBAR && nv <= 8; }
+#ifndef HX_T2_ONEBAR_NV
+#define HX_T2_ONEBAR_NV 8    // nvar 9 would fit with two z chunks, but their overhead eats the gain (wedge_3d 7.317 -> 7.303 ms, wedge_3d_rad 13.69 -> 13.97)
+#endif
+constexpr bool one_barrier(int nv) { return HX_T2_ONEBAR && nv <= HX_T2_ONEBAR_NV; }
 
 template <int NV, int TY>
 struct Smem {
@@ -104,7 +109,7 @@ struct Smem {
   static constexpr size_t plane_bytes = (size_t)NV * FSTR * sizeof(double);
   static constexpr size_t plane_stride = (plane_bytes + 127) / 128 * 128;
   static constexpr int NPL = 3;
-  static constexpr int XP = TX + 2;                            // x-exchange row pitch: slots ex = -1 .. TX-1 (+1 pad)
+  static constexpr int XP = TX + 1;                            // x-exchange row pitch: slots ex = -1 .. TX-1 (odd pitch: conflict-free columns)
   static constexpr int XSTR = TY * XP;                         // field stride of the x-exchange buffer
   static constexpr int YSTR = (TY + 1) * TX;                   // y-exchange: slots ey = -1 .. TY-1
   static constexpr size_t x_bytes = (size_t)NF * XSTR * sizeof(double);
@@ -118,8 +123,12 @@ struct Smem {
   // registers (they used to be spilled to local memory, which the 16 KB of L1 left beside the tile cannot hold)
   static constexpr int GT_X = TX + 2, GT_Y = TY + 2, NGX = 15, NGY = 12, GT_N = NGX * GT_X + NGY * GT_Y;
   static constexpr int XYSTR = NF * (XSTR + YSTR);             // doubles of one parity buffer (X fields, then Y fields)
-  static constexpr size_t fixed = NPL * plane_stride + NXY * (x_bytes + y_bytes) + priv_bytes + GT_N * sizeof(double) + 64 + 128;
-  static constexpr size_t total(int zc) { return fixed + 6 * (size_t)(zc + 6) * sizeof(double); }   // + z tables of one chunk
+  static constexpr size_t fixed = NPL * plane_stride + NXY * (x_bytes + y_bytes) + priv_bytes + 64 + 128;
+  // + the column / row factor tables (spherical builds) + the z tables of one chunk: hw, idx, dS-/dV, dS+/dV, g, 1/l along z;
+  // in spherical geometry dS-/dV, dS+/dV and 1/l are one and the same table (1 / dphi), stored once, and there is no
+  // acceleration along phi (uniform gravity on a spherical grid runs on the generic kernel)
+  static constexpr int nzt(bool sph) { return sph ? 3 : 6; }
+  static constexpr size_t total(int zc, bool sph) { return fixed + (sph ? GT_N * sizeof(double) : 0) + nzt(sph) * (size_t)(zc + 6) * sizeof(double); }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -702,7 +711,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   uint64_t* mbar = (uint64_t*)(XY0 + SM::NXY * SM::XYSTR);
   double* priv = (double*)(mbar + 8) + (threadIdx.x & (TY * TX - 1));   // private slots of the owner threads, field stride TY*TX
   double* gtab = (double*)(mbar + 8) + SM::NPRIV * TY * TX;   // spherical builds: column / row factor tables
-  double* zt = gtab + SM::GT_N;   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
+  double* zt = gtab + (SPH ? SM::GT_N : 0);   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
 
   const StepArgs& s = a.s;
   const Layout& L = s.L;
@@ -805,9 +814,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     zt[q] = T.hw[2][pz];
     zt[zlen + q] = T.idx[2][pz];
     zt[2 * zlen + q] = T.cf[2][0][2][pz];
-    zt[3 * zlen + q] = T.cf[2][1][2][pz];
-    zt[4 * zlen + q] = T.grav[2][pz];
-    zt[5 * zlen + q] = T.lf[2][2][pz];
+    if (!SPH) {   // spherical: cf[2][1][2] and lf[2][2] are the same table as cf[2][0][2] (1 / dphi); no acceleration along phi
+      zt[3 * zlen + q] = T.grav[2][pz];
+      zt[4 * zlen + q] = T.cf[2][1][2][pz];
+      zt[5 * zlen + q] = T.lf[2][2][pz];
+    }
   }
   if (GTAB) {   // column factors (with the (1 -+ rr) of Eq. 14) and row factors (with (1 -+ st)), (dt/2) folded in
     for (int e = threadIdx.x; e < SM::GT_X; e += blockDim.x) {
@@ -849,7 +860,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       g[11 * SM::GT_Y] = hdt * T.grav[1][pe];               // hgy
     }
   }
-  auto ZT = [&](int k, int pz) { return zt[k * zlen + (pz - zb)]; };
+  // table k of the list above at padded z index pz (k: 0 hw, 1 idx, 2 dS-/dV, 3 dS+/dV, 4 g, 5 1/l)
+  auto ZT = [&](int k, int pz) {
+    const int slot = SPH ? (k >= 2 ? 2 : k) : (k == 3 ? 4 : (k == 4 ? 3 : k));
+    return zt[slot * zlen + (pz - zb)];
+  };
   auto GX = [&](int k) { return gtab[k * SM::GT_X + ex + 1]; };                       // column factor k of this thread's cell
   auto GY = [&](int k) { return gtab[SM::NGX * SM::GT_X + k * SM::GT_Y + ey + 1]; };   // row factor k
   // the loop-invariant coefficients of this thread's column: table reads at use (GTAB) or the registers set up above
@@ -1040,7 +1055,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
       dU[2] = fma(rho, HGY(), dU[2]);
       dU[4] = fma(mcy, HGY(), dU[4]);
     }
-    if (grav_has(GRAV, 2)) {
+    if (grav_has(GRAV, 2, SPH)) {
       const double hgz = hdt * ZT(4, pk);
       dU[3] = fma(rho, hgz, dU[3]);
       dU[4] = fma(mcz, hgz, dU[4]);
@@ -1256,7 +1271,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
             Unew[4] = fma(Unm[1] + m2, HGY(), Unew[4]);
             Unew[2] = m2;
           }
-          if (grav_has(GRAV, 2)) {
+          if (grav_has(GRAV, 2, SPH)) {
             const double hgzp = hdt * ZT(4, pk - 1);
             const double m3 = fma(rs, hgzp, Unew[3]);
             Unew[4] = fma(Unm[2] + m3, hgzp, Unew[4]);
@@ -1299,7 +1314,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
           Un0 = Un[0];
           if (grav_has(GRAV, 0)) Unm[0] = Un[1];
           if (grav_has(GRAV, 1)) Unm[1] = Un[2];
-          if (grav_has(GRAV, 2)) Unm[2] = Un[3];
+          if (grav_has(GRAV, 2, SPH)) Unm[2] = Un[3];
         }
         if (EMON) {
           EA = fma(k2m, phz, fma(K.m0, phx, K.m1 * phy));

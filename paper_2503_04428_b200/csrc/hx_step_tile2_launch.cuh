@@ -29,7 +29,7 @@ template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EO
 static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   constexpr int TY = TY_DEFAULT;
   auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY, EOS, EMON>;
-  const size_t smem = Smem<NV, TY>::total(plan.zc);
+  const size_t smem = Smem<NV, TY>::total(plan.zc, SPH);
   cudaError_t e = set_smem_limit((const void*)kern, smem);
   if (e != cudaSuccess) return e;
   plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
