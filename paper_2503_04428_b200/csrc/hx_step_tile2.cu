@@ -156,7 +156,7 @@ cudaError_t launch_step_tile2(Plan* plan, const StepArgs& s, int cur, cudaStream
   a.zc = plan->zc;
   const double hdt = 0.5 * s.dt;
   for (int d = 0; d < 3; ++d) {
-    a.uf[d] = plan->uf[d] * (s.P.limiter == HX_LIM_MC ? 0.5 : 1.0);   // lim_scale of the specialised UNI build
+    a.uf[d] = plan->uf[d];                                             // (launch_cfg folds in the lim_scale of a static limiter)
     a.uhc[d] = hdt * plan->uiw[d];
     a.uil[d] = plan->uiw[d];
   }

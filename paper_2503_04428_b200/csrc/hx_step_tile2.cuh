@@ -77,7 +77,7 @@ struct Args {
   StepArgs s;
   int zc;            // planes per z chunk
   // UNI instantiations only (bitwise-uniform Cartesian tables): constants of the three axes
-  double uf[3];      // hw * idx   (slope pre-scale, = 1/2 up to rounding), times the limiter's lim_scale (1/2 for MC)
+  double uf[3];      // hw * idx   (slope pre-scale, = 1/2 up to rounding), times lim_scale of a build with a static limiter (1/2 for MC)
   double uhc[3];     // (dt/2) / delta_d
   double uil[3];     // 1 / delta_d  (CFL inverse lengths)
 };
@@ -199,6 +199,45 @@ __device__ __forceinline__ double lim_pre(int lim_rt, double dm, double dp, doub
   if (LIM == HX_LIM_NONE) return 0.0;
   if (UNI) return lim_core<LIM>(lim_rt, dm, dp);
   return lim_core<LIM>(lim_rt, dm * fl, dp * fh);
+}
+
+// N limited slopes at once: the runtime-switch builds (LIM < 0) branch ONCE on the warp-uniform limiter for all N
+// instead of once per slope (21-33 slopes per cell: the branches cost instructions and keep ptxas from interleaving the
+// slopes' chains).  fl / fh: one pre-scale pair for all (PER = false) or one per slope (PER = true).
+template <int N, int LIM, bool UNI, bool PER = false>
+__device__ __forceinline__ void lim_pre_n(int lim_rt, const double* dm, const double* dp, const double* fl, const double* fh, double* t) {
+  if (LIM >= 0) {
+#pragma unroll
+    for (int v = 0; v < N; ++v) t[v] = lim_pre<LIM, UNI>(lim_rt, dm[v], dp[v], fl[PER ? v : 0], fh[PER ? v : 0]);
+    return;
+  }
+  double a[N], b[N];
+#pragma unroll
+  for (int v = 0; v < N; ++v) {   // uniform grids: the common factor is left to the caller's face-state FMA (as in lim_pre)
+    a[v] = UNI ? dm[v] : dm[v] * fl[PER ? v : 0];
+    b[v] = UNI ? dp[v] : dp[v] * fh[PER ? v : 0];
+  }
+  switch (lim_rt) {
+    case HX_LIM_MINMOD:
+#pragma unroll
+      for (int v = 0; v < N; ++v) t[v] = lim_core<HX_LIM_MINMOD>(0, a[v], b[v]);
+      break;
+    case HX_LIM_MC:
+#pragma unroll
+      for (int v = 0; v < N; ++v) t[v] = 0.5 * lim_core<HX_LIM_MC>(0, a[v], b[v]);
+      break;
+    case HX_LIM_VANLEER:
+#pragma unroll
+      for (int v = 0; v < N; ++v) t[v] = lim_core<HX_LIM_VANLEER>(0, a[v], b[v]);
+      break;
+    case HX_LIM_VANALBADA:
+#pragma unroll
+      for (int v = 0; v < N; ++v) t[v] = lim_core<HX_LIM_VANALBADA>(0, a[v], b[v]);
+      break;
+    default:
+#pragma unroll
+      for (int v = 0; v < N; ++v) t[v] = 0.0;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1004,25 +1043,56 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     double uncl[6], pfl[6];     // gas + radiation EOS: per face (dt/2) dS/dV u_n and the face pressure
     double* const ul = unc6 ? unc6 : uncl;
     constexpr bool GR = EOS != HX_EOS_IDEAL;
+    double dm[NVP], dp[NVP];    // one-sided differences of a direction (runtime-switch builds: all slopes of a direction behind one branch)
+    if constexpr (LIM >= 0) {
 #pragma unroll
-    for (int v = 0; v < NVP; ++v) {
-      const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLX(), FHX());
+      for (int v = 0; v < NVP; ++v) {
+        const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
+        t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLX(), FHX());
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < NVP; ++v) {
+        const double wm = Pc[v * FSTR + cidx - 1], wp = Pc[v * FSTR + cidx + 1];
+        dm[v] = Wc[v] - wm;
+        dp[v] = wp - Wc[v];
+      }
+      const double fl = FLX(), fh = FHX();
+      lim_pre_n<NVP, LIM, UNI>(P.limiter, dm, dp, &fl, &fh, t);
     }
     face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? -FLX() : -lim_scale<LIM>(), HCM0(), Uxm, dU, (unc6 || GR) ? ul + 0 : nullptr, pfl + 0);
     face_cons_flux<NVP, 0, EOS>(P, Wc, t, UNI ? FLX() : lim_scale<LIM>(), -HCP0(), Uxp, dU, (unc6 || GR) ? ul + 1 : nullptr, pfl + 1);
+    if constexpr (LIM >= 0) {
 #pragma unroll
-    for (int v = 0; v < NVP; ++v) {
-      const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLY(), FHY());
+      for (int v = 0; v < NVP; ++v) {
+        const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
+        t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], FLY(), FHY());
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < NVP; ++v) {
+        const double wm = Pc[v * FSTR + cidx - PX], wp = Pc[v * FSTR + cidx + PX];
+        dm[v] = Wc[v] - wm;
+        dp[v] = wp - Wc[v];
+      }
+      const double fl = FLY(), fh = FHY();
+      lim_pre_n<NVP, LIM, UNI>(P.limiter, dm, dp, &fl, &fh, t);
     }
     face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? -FLY() : -lim_scale<LIM>(), HCM1(), Uym, dU, (unc6 || GR) ? ul + 2 : nullptr, pfl + 2);
     face_cons_flux<NVP, 1, EOS>(P, Wc, t, UNI ? FLY() : lim_scale<LIM>(), -HCP1(), Uyp, dU, (unc6 || GR) ? ul + 3 : nullptr, pfl + 3);
+    if constexpr (LIM >= 0) {
 #pragma unroll
-    for (int v = 0; v < NVP; ++v) {
-      const double dp = Wn[v] - Wc[v];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dp, flz, fhz);
-      dzm[v] = dp;
+      for (int v = 0; v < NVP; ++v) {
+        const double dpz = Wn[v] - Wc[v];
+        t[v] = lim_pre<LIM, UNI>(P.limiter, dzm[v], dpz, flz, fhz);
+        dzm[v] = dpz;
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < NVP; ++v) dp[v] = Wn[v] - Wc[v];
+      lim_pre_n<NVP, LIM, UNI>(P.limiter, dzm, dp, &flz, &fhz, t);
+#pragma unroll
+      for (int v = 0; v < NVP; ++v) dzm[v] = dp[v];
     }
     face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? -flz : -lim_scale<LIM>(), hcm2, Uzm, dU, (unc6 || GR) ? ul + 4 : nullptr, pfl + 4);
     face_cons_flux<NVP, 2, EOS>(P, Wc, t, UNI ? flz : lim_scale<LIM>(), -hcp2, Uzp, dU, (unc6 || GR) ? ul + 5 : nullptr, pfl + 5);
@@ -1143,10 +1213,19 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         for (int sv = 5; sv < NV; ++sv) {
           const double* Ps = Pc + sv * FSTR + cidx;
           const double fc = Ps[0];
-          const double tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, FLX(), FHX());
-          const double ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, FLY(), FHY());
           const double dp = Pn[sv * FSTR + cidx] - fc;
-          const double tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
+          double tx, ty, tz;
+          if constexpr (LIM >= 0) {
+            tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, FLX(), FHX());
+            ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, FLY(), FHY());
+            tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
+          } else {
+            const double dm3[3] = {fc - Ps[-1], fc - Ps[-PX], dzm[sv]}, dp3[3] = {Ps[1] - fc, Ps[PX] - fc, dp};
+            const double fl3[3] = {FLX(), FLY(), flz}, fh3[3] = {FHX(), FHY(), fhz};
+            double t3[3];
+            lim_pre_n<3, LIM, UNI, true>(P.limiter, dm3, dp3, fl3, fh3, t3);
+            tx = t3[0], ty = t3[1], tz = t3[2];
+          }
           dzm[sv] = dp;
           double rf[6];
           rf[0] = Uf[0][0] * fma(-scx, tx, fc);
@@ -1359,10 +1438,19 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         for (int sv = 5; sv < NV; ++sv) {
           const double* Ps = Pc + sv * FSTR + cidx;
           const double fc = Ps[0];
-          const double tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, FLX(), FHX());
-          const double ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, FLY(), FHY());
           const double dp = Pn[sv * FSTR + cidx] - fc;
-          const double tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
+          double tx, ty, tz;
+          if constexpr (LIM >= 0) {
+            tx = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-1], Ps[1] - fc, FLX(), FHX());
+            ty = lim_pre<LIM, UNI>(P.limiter, fc - Ps[-PX], Ps[PX] - fc, FLY(), FHY());
+            tz = lim_pre<LIM, UNI>(P.limiter, dzm[sv], dp, flz, fhz);
+          } else {
+            const double dm3[3] = {fc - Ps[-1], fc - Ps[-PX], dzm[sv]}, dp3[3] = {Ps[1] - fc, Ps[PX] - fc, dp};
+            const double fl3[3] = {FLX(), FLY(), flz}, fh3[3] = {FHX(), FHY(), fhz};
+            double t3[3];
+            lim_pre_n<3, LIM, UNI, true>(P.limiter, dm3, dp3, fl3, fh3, t3);
+            tx = t3[0], ty = t3[1], tz = t3[2];
+          }
           dzm[sv] = dp;
           double rf[6];
           rf[0] = Uf[0][0] * fma(-scx, tx, fc);

@@ -26,8 +26,11 @@ cudaError_t launch_nv(Plan& plan, const Args& a, int cur, cudaStream_t st);
 cudaError_t set_smem_limit(const void* kern, size_t smem);
 
 template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EOS_IDEAL, bool EMON = false>
-static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+static cudaError_t launch_cfg(Plan& plan, const Args& a_in, int cur, cudaStream_t st) {
   constexpr int TY = TY_DEFAULT;
+  Args a = a_in;
+  if (UNI && LIM == HX_LIM_MC)   // a build with a static limiter folds its lim_scale (1/2 for MC) into the uniform slope pre-scale
+    for (int d = 0; d < 3; ++d) a.uf[d] *= 0.5;
   auto kern = step_tile2_kernel<NV, SPH, GRAV, LIM, RS, UNI, TY, EOS, EMON>;
   const size_t smem = Smem<NV, TY>::total(plan.zc, SPH);
   cudaError_t e = set_smem_limit((const void*)kern, smem);
@@ -41,6 +44,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t s
 template <int NV, bool EMON = false>
 static cudaError_t launch_generic(Plan& plan, const Args& a, int cur, cudaStream_t st) {
   if (a.s.P.spherical) return launch_cfg<NV, true, GRAV_ANY, -1, -1, false, HX_EOS_IDEAL, EMON>(plan, a, cur, st);
+  if (plan.uni && !EMON) return launch_cfg<NV, false, GRAV_ANY, -1, -1, true, HX_EOS_IDEAL, EMON>(plan, a, cur, st);   // bitwise-uniform Cartesian grid
   return launch_cfg<NV, false, GRAV_ANY, -1, -1, false, HX_EOS_IDEAL, EMON>(plan, a, cur, st);
 }
 

@@ -80,8 +80,11 @@ cudaError_t tile2d_plan_fill(Plan* p, const Layout& L, double* const U[2], const
 namespace t2d {
 
 template <int NV, int GRAV, int LIM, int RS, bool UNI>
-static cudaError_t launch_cfg(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+static cudaError_t launch_cfg(Plan& plan, const Args& a_in, int cur, cudaStream_t st) {
   auto kern = step_tile2d_kernel<NV, GRAV, LIM, RS, UNI>;
+  Args a = a_in;
+  if (UNI && LIM == HX_LIM_MC)   // a build with a static limiter folds its lim_scale (1/2 for MC) into the uniform slope pre-scale
+    for (int d = 0; d < 2; ++d) a.uf[d] *= 0.5;
   const size_t smem = Smem<NV>::total(plan.zc);
   cudaError_t e = t2::set_smem_limit((const void*)kern, smem);
   if (e != cudaSuccess) return e;
@@ -98,7 +101,8 @@ static cudaError_t launch_nv(Plan& plan, const Args& a, int cur, cudaStream_t st
     if (P.limiter == HX_LIM_MC) return launch_cfg<NV, GRAV_OFF, HX_LIM_MC, HX_RIEMANN_HLLC, true>(plan, a, cur, st);
     if (P.limiter == HX_LIM_MINMOD) return launch_cfg<NV, GRAV_OFF, HX_LIM_MINMOD, HX_RIEMANN_HLLC, true>(plan, a, cur, st);
   }
-  return launch_cfg<NV, GRAV_ANY, -1, -1, false>(plan, a, cur, st);   // runtime switch: limiter, solver, gravity, any Cartesian grid
+  if (plan.uni) return launch_cfg<NV, GRAV_ANY, -1, -1, true>(plan, a, cur, st);   // runtime switch (limiter, solver, gravity) on a bitwise-uniform grid
+  return launch_cfg<NV, GRAV_ANY, -1, -1, false>(plan, a, cur, st);   // ... on any Cartesian grid
 }
 
 }  // namespace t2d
@@ -109,7 +113,7 @@ cudaError_t launch_step_tile2d(Plan* plan, const StepArgs& s, int cur, cudaStrea
   a.yc = plan->zc;
   const double hdt = 0.5 * s.dt;
   for (int d = 0; d < 2; ++d) {
-    a.uf[d] = plan->uf[d] * (s.P.limiter == HX_LIM_MC ? 0.5 : 1.0);   // lim_scale of the specialised UNI builds
+    a.uf[d] = plan->uf[d];                                             // (launch_cfg folds in the lim_scale of a static limiter)
     a.uhc[d] = hdt * plan->uiw[d];
     a.uil[d] = plan->uiw[d];
   }

@@ -30,6 +30,7 @@ namespace t2d {
 using t2::dmax;
 using t2::dmin;
 using t2::lim_pre;
+using t2::lim_pre_n;
 using t2::lim_scale;
 using t2::mbar_expect_tx;
 using t2::mbar_init;
@@ -442,22 +443,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) step_tile2d_kernel(const __grid_c
       fhy = hwy * YT(1, py + 1);
       hc1 = hdt * YT(2, py);
     }
-    double t[NV];
+    double t[NV], dm[NV], dp[NV];   // (runtime-switch builds: all slopes of a direction behind one branch on the limiter)
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       Wc[v] = Pc[v * HXS + cidx];
       dU[v] = 0.0;
       const double wm = Pc[v * HXS + cim], wp = Pc[v * HXS + cip];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, Wc[v] - wm, wp - Wc[v], flx, fhx);
+      dm[v] = Wc[v] - wm;
+      dp[v] = wp - Wc[v];
+      if constexpr (LIM >= 0) t[v] = lim_pre<LIM, UNI>(P.limiter, dm[v], dp[v], flx, fhx);
     }
+    if constexpr (LIM < 0) lim_pre_n<NV, LIM, UNI>(P.limiter, dm, dp, &flx, &fhx, t);
     face_cons_flux<NV, 0>(P, Wc, t, UNI ? -flx : -lim_scale<LIM>(), hc0, Uxm, dU);
     face_cons_flux<NV, 0>(P, Wc, t, UNI ? flx : lim_scale<LIM>(), -hc0, Uxp, dU);
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-      const double dp = Wn[v] - Wc[v];
-      t[v] = lim_pre<LIM, UNI>(P.limiter, dym[v], dp, fly, fhy);
-      dym[v] = dp;
+      dp[v] = Wn[v] - Wc[v];
+      if constexpr (LIM >= 0) t[v] = lim_pre<LIM, UNI>(P.limiter, dym[v], dp[v], fly, fhy);
     }
+    if constexpr (LIM < 0) lim_pre_n<NV, LIM, UNI>(P.limiter, dym, dp, &fly, &fhy, t);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) dym[v] = dp[v];
     face_cons_flux<NV, 1>(P, Wc, t, UNI ? -fly : -lim_scale<LIM>(), hc1, Uym, dU);
     face_cons_flux<NV, 1>(P, Wc, t, UNI ? fly : lim_scale<LIM>(), -hc1, Uyp, dU);
     if (GRAV == GRAV_ANY) {   // half step of rho g, m . g (R13)

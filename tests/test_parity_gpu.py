@@ -376,6 +376,29 @@ def test_uniform_grid_instantiations(hx, oxlib, name):
     assert max(l1) <= TOL_L1, (name, l1)
 
 
+@pytest.mark.parametrize("name,lim,riemann", [("rt_3d", wl.LIM_VANLEER, 1), ("rt_3d", wl.LIM_MINMOD, 0), ("sedov_3d", wl.LIM_MC, 1),
+                                              ("sedov_3d", wl.LIM_VANALBADA, 0), ("sedov_3d", wl.LIM_NONE, 1), ("kh_2d", wl.LIM_VANLEER, 1),
+                                              ("kh_2d", wl.LIM_MINMOD, 0), ("kh_2d", wl.LIM_NONE, 1)])
+def test_uniform_grid_runtime_switch_builds(hx, oxlib, name, lim, riemann):
+    """Bitwise-uniform grids with a limiter / solver that has no specialised build: the runtime-switch instantiations
+    with constant geometry (their slope pre-scale carries no lim_scale, unlike the static MC builds)."""
+    ox = oxlib
+    spec, W = {"rt_3d": lambda: wl.rt_3d((32, 64, 64)), "sedov_3d": lambda: wl.sedov_3d((64, 32, 32)), "kh_2d": lambda: wl.kh_2d((512, 64))}[name]()
+    spec = dict(spec, limiter=lim, riemann=riemann)
+    g, o = make_pair(hx, ox, spec, W)
+    for s in range(12):
+        dt_g, dt_o = g.compute_dt(spec["cfl"]), o.compute_dt(spec["cfl"])
+        assert abs(dt_g - dt_o) <= 1e-10 * dt_o, (s, dt_g, dt_o)
+        g.step(dt_g)
+        o.step(dt_o)
+        if s == 0:
+            assert g.step_kernel == ("tile2d_uni" if name == "kh_2d" else "tile2_uni"), g.step_kernel
+            rel = max_rel_per_field(g.get_state(), o.get_state(), spec["ndim"])
+            assert max(rel) <= TOL_STEP, (name, rel)
+    l1 = l1_rel_per_field(g.get_state(), o.get_state(), spec["ndim"])
+    assert max(l1) <= TOL_L1, (name, l1)
+
+
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times --------------------------------
 # (workload, expected step kernel, steps the GPU advances before the compared step: 0 = the initial state, 20 = a
 # late state in which the limiter and HLLC branches have switched on over the whole perturbed region)
