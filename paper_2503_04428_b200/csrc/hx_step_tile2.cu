@@ -47,8 +47,9 @@ static EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-static size_t smem_fixed(int nv) {   // shared memory of one CTA without the z tables of its chunk
+static size_t smem_fixed(int nv, int ty) {   // shared memory of one CTA without the z tables of its chunk
   constexpr int TY = t2::TY_DEFAULT;
+  if (ty == 12) return nv == 5 ? t2::Smem<5, 12>::fixed : 0;
   switch (nv) {
     case 5: return t2::Smem<5, TY>::fixed;
     case 6: return t2::Smem<6, TY>::fixed;
@@ -89,7 +90,8 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2]
     return cudaSuccess;
   }
   p->ndim = 3;
-  constexpr int TY = t2::TY_DEFAULT;
+  const int TY = t2::tile_rows(L, P, uni != nullptr);
+  p->ty = TY;
   const int ntx = (L.n[0] + t2::TX - 1) / t2::TX, nty = (L.n[1] + TY - 1) / TY;
   // z chunks: every chunk re-reads 4 planes and recomputes 2 predictor planes (+ a prologue), and with one CTA per
   // SM the grid runs in waves of `sms` CTAs of equal length: pick the chunk count that maximises
@@ -104,7 +106,7 @@ cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2]
   const long long cols = (long long)ntx * nty;
   // the chunk's z tables live in shared memory next to the plane ring and the exchange buffers (227 KB per CTA)
   constexpr int TYs = t2::TY_DEFAULT;
-  const size_t fixed = smem_fixed(L.nvar) + (P.spherical ? (size_t)t2::Smem<5, TYs>::GT_N * 8 : 0);   // (GT_N does not depend on the field count)
+  const size_t fixed = smem_fixed(L.nvar, TY) + (P.spherical ? (size_t)t2::Smem<5, TYs>::GT_N * 8 : 0);   // (GT_N does not depend on the field count)
   const size_t var_per_plane = (size_t)t2::Smem<5, TYs>::nzt(P.spherical != 0) * 8;
   const size_t budget = 227 * 1024 - 256;    // 256 B of static shared memory: the block reduction of the CFL rate
   int nzc = (L.n[2] + 15) / 16;

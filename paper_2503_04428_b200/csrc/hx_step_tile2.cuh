@@ -47,7 +47,7 @@ constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows (two warpgroups) + 4 ring
 // Register budgets after setmaxnreg.  The pool is what the CTA was given at launch, (TY+4) warps x 32 x REGS_LAUNCH
 // (not the whole 64 K file): the owners' increase must fit into what the ring warpgroup releases, or
 // setmaxnreg.inc waits forever.
-// Measured (A/B on B200): ring 96..120 is equal for the Cartesian builds.  The spherical ring path used to need 136
+// Measured (A/B on B200): ring 96..120 is equal for the Cartesian builds (96 with twelve owner rows).  The spherical ring path used to need 136
 // (nine fields at once, per-thread geometry products); with the scalars advanced one at a time (RING2) and the geometry
 // read from the shared column / row tables it runs in 120 like the Cartesian one from eight fields on (wedge_3d, nvar 9:
 // 104 -> 7.78 ms, 120 -> 7.31, 136 -> 7.51); the nvar 5-7 spherical builds keep 136 (sedov_wedge_3d: 1.14 vs 1.18 ms).
@@ -55,18 +55,19 @@ constexpr int TY_DEFAULT = HX_T2_TY;   // 8 owner rows (two warpgroups) + 4 ring
 #define HX_T2_REGS_RING_SPH 120
 #endif
 #ifdef HX_T2_REGS_RING
-constexpr int ring_regs(bool, int) { return HX_T2_REGS_RING; }
+constexpr int ring_regs(bool, int, int = TY_DEFAULT) { return HX_T2_REGS_RING; }
 #else
-constexpr int ring_regs(bool sph, int nv) { return (sph && nv < 8) ? 136 : (sph ? HX_T2_REGS_RING_SPH : 120); }
+constexpr int ring_regs(bool sph, int nv, int ty = TY_DEFAULT) { return ty > 8 ? 96 : ((sph && nv < 8) ? 136 : (sph ? HX_T2_REGS_RING_SPH : 120)); }
 #endif
-constexpr int REGS_LAUNCH = (65536 / ((TY_DEFAULT + 4) * 32)) / 8 * 8;
-constexpr int owner_regs(bool sph, int nv) {
-  const int raw = (REGS_LAUNCH * (TY_DEFAULT + 4) - ring_regs(sph, nv) * 4) / TY_DEFAULT / 8 * 8;
+constexpr int regs_launch(int ty) { return (65536 / ((ty + 4) * 32)) / 8 * 8; }
+constexpr int owner_regs(bool sph, int nv, int ty = TY_DEFAULT) {
+  const int raw = (regs_launch(ty) * (ty + 4) - ring_regs(sph, nv, ty) * 4) / ty / 8 * 8;
   return raw > 232 ? 232 : raw;
 }
-static_assert(owner_regs(true, 5) * TY_DEFAULT + ring_regs(true, 5) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
-static_assert(owner_regs(true, 9) * TY_DEFAULT + ring_regs(true, 9) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
-static_assert(owner_regs(false, 5) * TY_DEFAULT + ring_regs(false, 5) * 4 <= REGS_LAUNCH * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(true, 5) * TY_DEFAULT + ring_regs(true, 5) * 4 <= regs_launch(TY_DEFAULT) * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(true, 9) * TY_DEFAULT + ring_regs(true, 9) * 4 <= regs_launch(TY_DEFAULT) * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(false, 5) * TY_DEFAULT + ring_regs(false, 5) * 4 <= regs_launch(TY_DEFAULT) * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
+static_assert(owner_regs(false, 5, 12) * 12 + ring_regs(false, 5, 12) * 4 <= regs_launch(12) * 16, "setmaxnreg budgets exceed the launch allocation");
 
 enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2, GRAV_R = 3 };   // GRAV_Z / GRAV_R: acceleration along direction 2 / 0 only (uniform g along z; point mass, self-gravity)
 constexpr bool grav_has(int grav, int d, bool sph = false) {
@@ -748,7 +749,7 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   constexpr bool RING2 = NV >= HX_T2_RING2_NV;   // ring warps: hydro fields first, then the passive scalars one at a time
   double* const XY0 = (double*)(base + SM::NPL * SM::plane_stride);   // parity buffer 0: X fields, then Y fields; buffer 1 follows (ONEBAR)
   uint64_t* mbar = (uint64_t*)(XY0 + SM::NXY * SM::XYSTR);
-  double* priv = (double*)(mbar + 8) + (threadIdx.x & (TY * TX - 1));   // private slots of the owner threads, field stride TY*TX
+  double* priv = (double*)(mbar + 8) + min((int)threadIdx.x, TY * TX - 1);   // private slots of the owner threads, field stride TY*TX
   double* gtab = (double*)(mbar + 8) + SM::NPRIV * TY * TX;   // spherical builds: column / row factor tables
   double* zt = gtab + (SPH ? SM::GT_N : 0);   // z-axis tables of this chunk, staged once (per-plane global loads stall the march)
 
@@ -1529,11 +1530,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   }
   };
   if (owner) {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(owner_regs(SPH, NV)));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(owner_regs(SPH, NV, TY)));
     march(std::true_type{});
     cfl_rate(k1 + 1 + NG - 2);                           // the last cell written (plane k1-1)
   } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ring_regs(SPH, NV)));
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ring_regs(SPH, NV, TY)));
     march(std::false_type{});
   }
 

@@ -10,6 +10,7 @@ struct Plan {
   CUtensorMap tmap[2];
   int ndim;          // 3: hx_step_tile2.cuh (march along z); 2: hx_step_tile2d.cuh (march along y)
   int zc;            // planes (rows in 2-D) per chunk of the march direction
+  int ty;            // owner rows of a 3-D tile: 8, or 12 for the configuration tile_rows() names
   dim3 grid;
   bool uni;          // bitwise-uniform Cartesian tables: geometry travels as kernel-parameter constants
   bool grav_z;       // uniform gravity along direction 2 only
@@ -25,9 +26,20 @@ cudaError_t launch_nv(Plan& plan, const Args& a, int cur, cudaStream_t st);
 // (kernel, device), under a lock -- handles of one process may live on several GPUs and step from several threads.
 cudaError_t set_smem_limit(const void* kern, size_t smem);
 
-template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EOS_IDEAL, bool EMON = false>
+// Owner rows per tile.  Twelve rows (three owner warps + one ring warp per scheduler, 136 registers per owner thread) carry less
+// ring work per cell; they pay only where the owner path fits into those registers: nvar 5, Cartesian, constant geometry, no
+// gravity, minmod + HLLC (config 3: sedov_3d 0.970 -> 0.936 ms; nvar 7 spills and needs two z chunks: 10.30 -> 12.69 ms;
+// the spherical nvar-5 build: 1.11 -> 1.22 ms).  One place decides, for the plan (grid, shared memory) and for the dispatch.
+inline int tile_rows(const Layout& L, const Phys& P, bool uni) {
+  const bool c3 = L.nvar == 5 && !P.spherical && uni && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC &&
+                  P.eos == HX_EOS_IDEAL && !(P.emon_eps > 0.0) && L.n[1] >= 24 &&
+                  ((L.n[1] + 11) / 12 * 12 - L.n[1]) * 25 <= L.n[1];   // at most 4 % of the tile rows beyond the grid
+  return c3 ? 12 : TY_DEFAULT;
+}
+
+template <int NV, bool SPH, int GRAV, int LIM, int RS, bool UNI, int EOS = HX_EOS_IDEAL, bool EMON = false, int TY = TY_DEFAULT>
 static cudaError_t launch_cfg(Plan& plan, const Args& a_in, int cur, cudaStream_t st) {
-  constexpr int TY = TY_DEFAULT;
+  if (plan.ty != TY) return cudaErrorInvalidConfiguration;   // the plan's grid and shared memory were sized for another tile height
   Args a = a_in;
   if (UNI && LIM == HX_LIM_MC)   // a build with a static limiter folds its lim_scale (1/2 for MC) into the uniform slope pre-scale
     for (int d = 0; d < 3; ++d) a.uf[d] *= 0.5;
@@ -35,7 +47,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a_in, int cur, cudaStream_
   const size_t smem = Smem<NV, TY>::total(plan.zc, SPH);
   cudaError_t e = set_smem_limit((const void*)kern, smem);
   if (e != cudaSuccess) return e;
-  plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? "tile2_uni" : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
+  plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? (TY == 12 ? "tile2_uni12" : "tile2_uni") : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
   kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();
 }

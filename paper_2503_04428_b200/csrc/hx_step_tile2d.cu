@@ -57,6 +57,7 @@ cudaError_t tile2d_plan_fill(Plan* p, const Layout& L, double* const U[2], const
   const int nyc = (L.n[1] + p->zc - 1) / p->zc;
   p->grid = dim3((unsigned)ntx, (unsigned)nyc, 1u);
   p->ndim = 2;
+  p->ty = 0;
   p->uni = uni != nullptr;
   p->grav_z = false;
   p->grav_r = false;

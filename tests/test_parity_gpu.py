@@ -355,6 +355,7 @@ UNIFORM = {   # 2^k cells on dyadic extents: bitwise-uniform tables -> the const
     "sedov_3d": lambda: wl.sedov_3d((64, 32, 32)),
     "rt_3d": lambda: wl.rt_3d((32, 64, 64)),
     "cold_stream_3d": lambda: wl.cold_stream_3d((64, 32, 32)),   # internal-energy monitoring in the tile kernel
+    "sedov_3d_rows12": lambda: wl.sedov_3d((64, 128, 32)),       # config 3's own build: twelve owner rows per tile (n1 = 128 -> 11 tile rows)
 }
 
 
@@ -369,7 +370,7 @@ def test_uniform_grid_instantiations(hx, oxlib, name):
         g.step(dt_g)
         o.step(dt_o)
         if s == 0:
-            assert g.step_kernel == ("tile2_emon_uni" if name == "cold_stream_3d" else "tile2_uni")
+            assert g.step_kernel == {"cold_stream_3d": "tile2_emon_uni", "sedov_3d_rows12": "tile2_uni12"}.get(name, "tile2_uni")
             rel = max_rel_per_field(g.get_state(), o.get_state(), 3)
             assert max(rel) <= TOL_STEP, (name, rel)
     l1 = l1_rel_per_field(g.get_state(), o.get_state(), 3)
@@ -403,7 +404,7 @@ def test_uniform_grid_runtime_switch_builds(hx, oxlib, name, lim, riemann):
 # (workload, expected step kernel, steps the GPU advances before the compared step: 0 = the initial state, 20 = a
 # late state in which the limiter and HLLC branches have switched on over the whole perturbed region)
 FULL = {
-    "sedov_3d": (lambda: wl.sedov_3d(256), "tile2_uni", 0),
+    "sedov_3d": (lambda: wl.sedov_3d(256), "tile2_uni12", 0),
     "rt_3d": (lambda: wl.rt_3d(512), "tile2_uni", 0),
     "rt_3d_late": (lambda: wl.rt_3d(512), "tile2_uni", 20),
     "wedge_3d": (lambda: wl.wedge_3d((1024, 256, 256)), "tile2", 0),
@@ -420,7 +421,7 @@ FULL = {
 
 def sample_cells(n, seed, extra):
     """Cells the oracle evaluates one by one: domain corners and face centres, both sides of tile edges
-    (x multiples of 32, y multiples of 8) and of z-chunk edges, cells where the workload has structure
+    (x multiples of 32, y multiples of 8 and of 12) and of z-chunk edges, cells where the workload has structure
     (`extra`), and seeded random interior cells."""
     nx, ny, nz = n
     rng = np.random.default_rng(seed)
@@ -429,8 +430,9 @@ def sample_cells(n, seed, extra):
         for j in (0, 1, ny // 2, ny - 2, ny - 1):
             for k in (0, 1, nz // 2, nz - 2, nz - 1):
                 cells.add((i, j, k))
-    for _ in range(60):
-        ti, tj = 32 * int(rng.integers(1, max(2, nx // 32))), 8 * int(rng.integers(1, max(2, ny // 8)))
+    for q in range(90):
+        th = 8 if q < 60 else 12                    # tile rows: 8, or 12 in the config-3 build
+        ti, tj = 32 * int(rng.integers(1, max(2, nx // 32))), th * int(rng.integers(1, max(2, ny // th)))
         k = int(rng.integers(0, nz))
         for di in (-1, 0):
             for dj in (-1, 0):
@@ -581,7 +583,7 @@ def test_full_size_ten_steps_sedov(hx, oxlib):
         assert abs(dt_g - dt_o) <= 1e-11 * dt_o, (s, dt_g, dt_o)
         g.step(dt_g)
         o.step(dt_o)
-    assert g.step_kernel == "tile2_uni"
+    assert g.step_kernel == "tile2_uni12"
     Ug, Uo = g.get_state(), o.get_state()
     assert max(l1_rel_per_field(Ug, Uo, 3)) <= TOL_L1
     assert max(max_rel_per_field(Ug, Uo, 3)) <= 1e-11
