@@ -107,10 +107,20 @@ cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, cons
 struct SelfGrav {
   const double* xf[3];   // padded face coordinates of the three axes (device)
   double* partial;       // [nrows_groups][n0]
+  const double* weights; // theta weights cos(th-) - cos(th+) [n1], then phi widths [n2] (constant in time: computed once)
   double* grav_r;        // the table T.grav[0], np[0] entries
   double GM, G;
   int groups, bc_lo, bc_hi;
 };
+
+__global__ void shell_weights_kernel(Layout L, SelfGrav sg, double* w) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < L.n[1]) w[t] = cos(sg.xf[1][t + L.ng[1]]) - cos(sg.xf[1][t + L.ng[1] + 1]);
+  else if (t < L.n[1] + L.n[2]) {
+    const int k = t - L.n[1];
+    w[t] = sg.xf[2][k + L.ng[2] + 1] - sg.xf[2][k + L.ng[2]];
+  }
+}
 
 __global__ void shell_mass_partial_kernel(Layout L, const double* __restrict__ U, SelfGrav sg) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -119,8 +129,7 @@ __global__ void shell_mass_partial_kernel(Layout L, const double* __restrict__ U
   double acc = 0.0;
   for (int r = blockIdx.y; r < rows; r += gridDim.y) {
     const int j = r % L.n[1], k = r / L.n[1];
-    const double wt = cos(sg.xf[1][j + L.ng[1]]) - cos(sg.xf[1][j + L.ng[1] + 1]);
-    const double wp = sg.xf[2][k + L.ng[2] + 1] - sg.xf[2][k + L.ng[2]];
+    const double wt = sg.weights[j], wp = sg.weights[L.n[1] + k];
     acc = fma(U[L.off(i + L.ng[0], j + L.ng[1], k + L.ng[2])], wt * wp, acc);
   }
   sg.partial[(size_t)blockIdx.y * L.n[0] + i] = acc;
@@ -165,11 +174,19 @@ __global__ void self_gravity_table_kernel(Layout L, SelfGrav sg) {
   }
 }
 
+// weights: n1 + n2 doubles of device memory; *weights_ready: filled on the first call (the angular weights do not change in time)
 cudaError_t launch_self_gravity(const Layout& L, const double* U, const double* const xf[3], double* partial, int groups, double* grav_r,
-                                double GM, double G, int bc_lo, int bc_hi, cudaStream_t s) {
+                                double GM, double G, int bc_lo, int bc_hi, double* weights, bool* weights_ready, cudaStream_t s) {
   SelfGrav sg;
   for (int d = 0; d < 3; ++d) sg.xf[d] = xf[d];
   sg.partial = partial;
+  sg.weights = weights;
+  if (!*weights_ready) {
+    const int nw = L.n[1] + L.n[2];
+    shell_weights_kernel<<<(nw + 255) / 256, 256, 0, s>>>(L, sg, weights);
+    if (cudaGetLastError() != cudaSuccess) return cudaErrorLaunchFailure;
+    *weights_ready = true;
+  }
   sg.grav_r = grav_r;
   sg.GM = GM;
   sg.G = G;

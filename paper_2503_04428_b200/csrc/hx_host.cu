@@ -17,7 +17,7 @@ cudaError_t launch_rate(const Layout& L, const Tables& T, const Phys& P, const d
                         cudaStream_t s);
 cudaError_t launch_step_generic(const StepArgs& a, cudaStream_t s);
 cudaError_t launch_self_gravity(const Layout& L, const double* U, const double* const xf[3], double* partial, int groups, double* grav_r,
-                                double GM, double G, int bc_lo, int bc_hi, cudaStream_t s);
+                                double GM, double G, int bc_lo, int bc_hi, double* weights, bool* weights_ready, cudaStream_t s);
 namespace t2 { struct Plan; }
 int tile2_supported(const Layout& L, const Phys& P);
 cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, t2::Plan** out);
@@ -49,7 +49,8 @@ struct hx_handle {
   cudaEvent_t ev_step = nullptr;  // recorded right after the step kernel
   const double* d_xf[3] = {nullptr, nullptr, nullptr};   // padded face coordinates on the device (self-gravity)
   double* d_grav_r = nullptr;     // the radial acceleration table inside d_tables (rewritten every step by self-gravity)
-  double* d_sg_partial = nullptr; // self-gravity: partial shell sums [sg_groups][n0]
+  double* d_sg_partial = nullptr; // self-gravity: partial shell sums [sg_groups][n0], then the angular weights [n1 + n2]
+  bool sg_weights_ready = false;
   int sg_groups = 0;
   bool ghosts_valid = false;      // ghost layers of d_U[cur] are filled (hx_step fills them eagerly for the next step)
   bool rate_valid = false;
@@ -388,7 +389,7 @@ int hx_create(const hx_config* cfg, hx_handle** out) {
   if (cfg->gravity == HX_GRAV_SELF) {
     const long long rows = (long long)L.n[1] * L.n[2];
     h->sg_groups = (int)(rows < 296 ? rows : 296);
-    if (cudaMalloc(&h->d_sg_partial, (size_t)h->sg_groups * L.n[0] * sizeof(double)) != cudaSuccess) { hx_destroy(h); return HX_ERR_ALLOC; }
+    if (cudaMalloc(&h->d_sg_partial, ((size_t)h->sg_groups * L.n[0] + L.n[1] + L.n[2]) * sizeof(double)) != cudaSuccess) { hx_destroy(h); return HX_ERR_ALLOC; }
   }
   h->cfg.faces[0] = h->cfg.faces[1] = h->cfg.faces[2] = nullptr;   // caller arrays are not retained
   *out = h;
@@ -559,7 +560,7 @@ int hx_step(hx_handle* h, double dt) {
   }
   if (h->cfg.gravity == HX_GRAV_SELF) {   // Eq. 4 from U^n: shell masses, scan over r, new radial acceleration table
     e = launch_self_gravity(L, h->d_U[h->cur], h->d_xf, h->d_sg_partial, h->sg_groups, h->d_grav_r, h->cfg.GM, h->cfg.G, h->cfg.bc_lo[0],
-                            h->cfg.bc_hi[0], h->stream);
+                            h->cfg.bc_hi[0], h->d_sg_partial + (size_t)h->sg_groups * L.n[0], &h->sg_weights_ready, h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: self-gravity");
     h->launches += 2;
   }
