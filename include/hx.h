@@ -123,6 +123,31 @@ int hx_kernel_time(hx_handle* h, double* total_ms, long long* launches);
  * GPU in TFLOP/s (1 FMA = 2 flop; many independent chains on every SM) and the issue-to-issue latency
  * of a dependent DFMA in SM cycles.  This is the denominator of the "alu" roofline. */
 int hx_probe_fp64(double* tflops, double* dep_latency_cycles);
+/* HX_GRAV_SELF handles only: refresh the radial acceleration table from the CURRENT state exactly as hx_step does before its
+ * step kernel (Eq. 4, R28; shell-mass reduction through the handle's cudaMalloc'ed scratch + scan) and copy its n[0]
+ * interior entries g_r(r_c,i) to out (HX_HOST or HX_DEVICE pointer).  Synchronises for a host pointer.  HX_ERR_UNSUPPORTED for
+ * other gravity types.  The cross-check of hx_self_gravity_noalloc below. */
+int hx_self_gravity_table(hx_handle* h, double* out, int mem_space);
+
+/* ---- entry point that allocates nothing (callers under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc) -- */
+/* The self-gravity refresh of Eq. 4 (R28) without a handle and without any device allocation:
+ *   g[i] = -( GM + G (4 pi / dOmega) ( sum_{i'<i} m_i' + m_i (r_c^3 - r_-^3)/(r_+^3 - r_-^3) ) ) / r_c^2,   i = 0 .. n0-1,
+ * m_i = sum_{j,k} rho dV the shell masses, dOmega the solid angle of the grid, r_c = (r_- + r_+)/2.
+ * ALL pointers are DEVICE pointers owned by the caller: rho = interior density [n2][n1][n0] (direction 0 fastest), faces_r /
+ * faces_theta / faces_phi = n0+1 / n1+1 / n2+1 increasing face coordinates, g = n0 outputs.  The partial shell sums (the scratch
+ * the handle path keeps in cudaMalloc'ed memory) live in a file-scope `static __device__` array of the library, 2 MiB + 32 KiB,
+ * which every GPU that loads libhx.so holds until the process exits.  Hence the limits: n0 <= HX_NOALLOC_MAX_N0 and
+ * n1 + n2 <= HX_NOALLOC_MAX_ANGULAR; larger sizes are rejected with HX_ERR_UNSUPPORTED (message from hx_noalloc_error()).
+ * The call enqueues three kernels on cuda_stream (a cudaStream_t, NULL = legacy default stream) and returns; it calls no
+ * cudaMalloc / cudaFree / allocating library routine and does not synchronise.  Every call on a GPU shares the one array: the
+ * array keeps the last call's contents (each call overwrites every entry it later reads, nothing needs to start at zero), and
+ * two calls that overlap on the GPU (different streams, different host threads) RACE on it -- serialise them. */
+#define HX_NOALLOC_MAX_N0 2048
+#define HX_NOALLOC_MAX_ANGULAR 4096
+int hx_self_gravity_noalloc(const double* rho, const double* faces_r, const double* faces_theta, const double* faces_phi, int n0, int n1,
+                            int n2, double GM, double G, double* g, void* cuda_stream);
+/* Message of the last failing hx_self_gravity_noalloc call of this host thread ("" if none). */
+const char* hx_noalloc_error(void);
 
 #ifdef __cplusplus
 }

@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 # HX_LIBRARY: load (and build into) another file, e.g. an A/B variant built with other -D flags
 LIB = os.environ.get("HX_LIBRARY") or os.path.join(HERE, "libhx.so")
-SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_probe.cu",
+SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_probe.cu", "hx_noalloc.cu",
            "hx_step_tile2.cu", "hx_step_tile2_nv5.cu", "hx_step_tile2_nv6.cu", "hx_step_tile2_nv7.cu", "hx_step_tile2_nv9.cu", "hx_step_tile2_nv9_rad.cu", "hx_step_tile2d.cu",
            "hx_step_tile2_nv8.cu", "hx_step_tile2_nv10.cu", "hx_step_tile2_nv11.cu", "hx_step_tile2_nv5_rad.cu", "hx_step_tile2_nv6_rad.cu",
            "hx_step_tile2_nv7_rad.cu", "hx_step_tile2_nv8_rad.cu", "hx_step_tile2_nv10_rad.cu", "hx_step_tile2_nv11_rad.cu"] + \

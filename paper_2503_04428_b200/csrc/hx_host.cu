@@ -548,6 +548,24 @@ int hx_compute_dt(hx_handle* h, double cfl, double* dt_out) {
   return HX_OK;
 }
 
+// Diagnostic: the handle path of the self-gravity refresh (the same launch hx_step makes), table read back.
+int hx_self_gravity_table(hx_handle* h, double* out, int mem_space) {
+  if (!h || !out) return HX_ERR_INVALID_ARG;
+  if (mem_space != HX_HOST && mem_space != HX_DEVICE) return fail(h, HX_ERR_INVALID_ARG, "bad mem_space");
+  if (h->cfg.gravity != HX_GRAV_SELF) return fail(h, HX_ERR_UNSUPPORTED, "hx_self_gravity_table needs HX_GRAV_SELF");
+  const Layout& L = h->L;
+  cudaError_t e = launch_self_gravity(L, h->d_U[h->cur], h->d_xf, h->d_sg_partial, h->sg_groups, h->d_grav_r, h->cfg.GM, h->cfg.G,
+                                      h->cfg.bc_lo[0], h->cfg.bc_hi[0], h->d_sg_partial + (size_t)h->sg_groups * L.n[0], &h->sg_weights_ready,
+                                      h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "hx_self_gravity_table: self-gravity");
+  h->launches += 2;
+  e = cudaMemcpyAsync(out, h->d_grav_r + L.ng[0], (size_t)L.n[0] * sizeof(double),
+                      mem_space == HX_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, h->stream);
+  if (e == cudaSuccess && mem_space == HX_HOST) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "hx_self_gravity_table: copy");
+  return HX_OK;
+}
+
 int hx_step(hx_handle* h, double dt) {
   if (!h) return HX_ERR_INVALID_ARG;
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, HX_ERR_INVALID_ARG, "dt must be positive and finite");

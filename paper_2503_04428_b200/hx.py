@@ -27,7 +27,8 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 EXPORTS = ["hx_create", "hx_destroy", "hx_set_stream", "hx_set_option", "hx_set_state", "hx_get_state",
            "hx_compute_dt", "hx_step", "hx_nvar", "hx_launch_count", "hx_kernel_time", "hx_step_kernel_name", "hx_last_error",
-           "hx_version", "hx_probe_fp64", "hx_config_size", "hx_sync"]
+           "hx_version", "hx_probe_fp64", "hx_config_size", "hx_sync", "hx_self_gravity_table", "hx_self_gravity_noalloc", "hx_noalloc_error"]
+NOALLOC_MAX_N0, NOALLOC_MAX_ANGULAR = 2048, 4096
 
 
 class HxConfig(C.Structure):
@@ -74,6 +75,9 @@ def lib():
         L.hx_compute_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
         L.hx_step.argtypes = [vp, C.c_double]
         L.hx_sync.argtypes = [vp]
+        L.hx_self_gravity_table.argtypes = [vp, dp, C.c_int]
+        L.hx_self_gravity_noalloc.argtypes = [dp, dp, dp, dp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, dp, vp]
+        L.hx_noalloc_error.restype = C.c_char_p
         L.hx_nvar.argtypes = [vp]
         L.hx_launch_count.argtypes = [vp]
         L.hx_launch_count.restype = C.c_longlong
@@ -208,6 +212,13 @@ class Hydro:
     def sync(self):
         self._check(self._L.hx_sync(self._h), "hx_sync")
 
+    def self_gravity_table(self):
+        """HX_GRAV_SELF handles: the n[0] interior radial accelerations g_r(r_c,i) of the current state, through the handle's
+        (cudaMalloc'ed) scratch -- the path hx_step uses."""
+        out = np.empty(self.n[0], dtype=np.float64)
+        self._check(self._L.hx_self_gravity_table(self._h, C.c_void_p(out.ctypes.data), HOST), "hx_self_gravity_table")
+        return out
+
     def kernel_time(self):
         """(total ms, launches) of the step kernel alone, measured with CUDA events (OPT_TIMING on)."""
         ms, cnt = C.c_double(), C.c_longlong()
@@ -221,6 +232,28 @@ class Hydro:
     @property
     def step_kernel(self) -> str:
         return self._L.hx_step_kernel_name(self._h).decode()
+
+
+def self_gravity_noalloc(rho, faces_r, faces_theta, faces_phi, GM, G, g, stream=None):
+    """hx_self_gravity_noalloc: the self-gravity refresh of Eq. 4 with no device allocation (scratch in a static __device__
+    array of the library).  All arrays are float64 CUDA tensors: rho [n2][n1][n0], the three face arrays, g [n0] (output).
+    Asynchronous on `stream` (default: the legacy default stream).  Sizes beyond NOALLOC_MAX_N0 / NOALLOC_MAX_ANGULAR raise
+    HxError(ERR_UNSUPPORTED)."""
+    n2, n1, n0 = (int(x) for x in rho.shape)
+    ptrs = []
+    for name, buf, count in (("rho", rho, n0 * n1 * n2), ("faces_r", faces_r, n0 + 1), ("faces_theta", faces_theta, n1 + 1),
+                             ("faces_phi", faces_phi, n2 + 1), ("g", g, n0)):
+        ptr, space, have = _pointer(buf)
+        if space != DEVICE:
+            raise TypeError(f"{name} must be a CUDA tensor")
+        if have != count:
+            raise ValueError(f"{name} has {have} elements, expected {count}")
+        ptrs.append(C.c_void_p(ptr))
+    sp = 0 if stream is None else (stream if isinstance(stream, int) else getattr(stream, "cuda_stream", 0))
+    L = lib()
+    rc = L.hx_self_gravity_noalloc(ptrs[0], ptrs[1], ptrs[2], ptrs[3], n0, n1, n2, float(GM), float(G), ptrs[4], C.c_void_p(sp))
+    if rc != OK:
+        raise HxError(rc, "hx_self_gravity_noalloc", L.hx_noalloc_error().decode())
 
 
 def probe_fp64():
