@@ -10,7 +10,7 @@
 #include "hx_common.cuh"
 
 namespace hx {
-cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, const int* bc_hi, cudaStream_t s);
+cudaError_t launch_ghost_fill(const Layout& L, double* U, const int* bc_lo, const int* bc_hi, int skip_x, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const Phys& P, const double* src, double* U, int to_cons, cudaStream_t s);
 cudaError_t launch_unpack(const Layout& L, const Phys& P, const double* U, double* dst, int to_prim, cudaStream_t s);
 cudaError_t launch_rate(const Layout& L, const Tables& T, const Phys& P, const double* U, unsigned long long* rate_bits, int* status,
@@ -20,7 +20,8 @@ cudaError_t launch_self_gravity(const Layout& L, const double* U, const double* 
                                 double GM, double G, int bc_lo, int bc_hi, double* weights, bool* weights_ready, cudaStream_t s);
 namespace t2 { struct Plan; }
 int tile2_supported(const Layout& L, const Phys& P);
-cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, t2::Plan** out);
+cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, int bcx_lo, int bcx_hi, t2::Plan** out);
+int tile2_writes_x_ghosts(const t2::Plan* p);
 void tile2_plan_destroy(t2::Plan* p);
 cudaError_t launch_step_tile2(t2::Plan* plan, const StepArgs& a, int cur, cudaStream_t s);
 const char* tile2_kernel_name(const t2::Plan* p);
@@ -572,7 +573,7 @@ int hx_step(hx_handle* h, double dt) {
   const Layout& L = h->L;
   cudaError_t e;
   if (!h->ghosts_valid) {   // A0: all directions, one launch (normally done eagerly at the end of the previous hx_step)
-    e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);
+    e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, 0, h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: ghost fill");
     h->launches++;
   }
@@ -591,7 +592,7 @@ int hx_step(hx_handle* h, double dt) {
     if (!h->plan2 && !h->plan2_tried) {
       h->plan2_tried = true;
       const int grav_z = h->cfg.gravity == HX_GRAV_UNIFORM && h->cfg.g[0] == 0.0 && h->cfg.g[1] == 0.0;
-      e = tile2_plan_create(L, h->P, h->d_U, h->uniform ? h->uni : nullptr, grav_z, &h->plan2);
+      e = tile2_plan_create(L, h->P, h->d_U, h->uniform ? h->uni : nullptr, grav_z, h->cfg.bc_lo[0], h->cfg.bc_hi[0], &h->plan2);
       if (e != cudaSuccess) {
         h->plan2 = nullptr;
         return cuda_fail(h, e, "hx_step: tile2 plan");   // no silent fallback to a slower path
@@ -620,7 +621,8 @@ int hx_step(hx_handle* h, double dt) {
   // The next step needs the ghost layers of the new state whatever its dt will be: fill them now, behind the event
   // hx_compute_dt waits for, so that the host's read-back of the CFL rate overlaps this kernel.
   e = cudaEventRecord(h->ev_step, h->stream);
-  if (e == cudaSuccess) e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, h->stream);
+  if (e == cudaSuccess)   // (the 3-D tile kernel has written the x-ghost cells of the interior rows itself)
+    e = launch_ghost_fill(L, h->d_U[h->cur], h->cfg.bc_lo, h->cfg.bc_hi, use_tile2 && tile2_writes_x_ghosts(h->plan2), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "hx_step: eager ghost fill");
   h->launches++;
   h->ghosts_valid = true;

@@ -75,11 +75,16 @@ int tile2_supported(const Layout& L, const Phys& P) {
 
 // uni: non-null when every per-axis table of this Cartesian grid is bitwise constant; then uni[0..2] = hw*idx and
 // uni[3..5] = 1/delta of the three axes.
-cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, Plan** out) {
+int tile2_writes_x_ghosts(const Plan* p) { return p && p->ndim == 3 && p->xghost; }   // valid after a launch
+
+cudaError_t tile2_plan_create(const Layout& L, const Phys& P, double* const U[2], const double* uni, int grav_z, int bcx_lo, int bcx_hi, Plan** out) {
   *out = nullptr;
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   Plan* p = new Plan();
+  p->xghost = false;
+  p->bcx_lo = bcx_lo;
+  p->bcx_hi = bcx_hi;
   if (L.ndim == 2) {
     cudaError_t e2 = tile2d_plan_fill(p, L, U, uni, (void*)enc);
     if (e2 != cudaSuccess) {
@@ -156,6 +161,8 @@ cudaError_t launch_step_tile2(Plan* plan, const StepArgs& s, int cur, cudaStream
   t2::Args a;
   a.s = s;
   a.zc = plan->zc;
+  a.bcx_lo = plan->bcx_lo;
+  a.bcx_hi = plan->bcx_hi;
   const double hdt = 0.5 * s.dt;
   for (int d = 0; d < 3; ++d) {
     a.uf[d] = plan->uf[d];                                             // (launch_cfg folds in the lim_scale of a static limiter)

@@ -69,6 +69,8 @@ static_assert(owner_regs(true, 9) * TY_DEFAULT + ring_regs(true, 9) * 4 <= regs_
 static_assert(owner_regs(false, 5) * TY_DEFAULT + ring_regs(false, 5) * 4 <= regs_launch(TY_DEFAULT) * (TY_DEFAULT + 4), "setmaxnreg budgets exceed the launch allocation");
 static_assert(owner_regs(false, 5, 12) * 12 + ring_regs(false, 5, 12) * 4 <= regs_launch(12) * 16, "setmaxnreg budgets exceed the launch allocation");
 
+constexpr bool writes_x_ghosts(bool uni, int ty) { return uni && ty == 8; }   // builds whose boundary threads also write the x-ghost cells
+
 enum { GRAV_OFF = 0, GRAV_ANY = 1, GRAV_Z = 2, GRAV_R = 3 };   // GRAV_Z / GRAV_R: acceleration along direction 2 / 0 only (uniform g along z; point mass, self-gravity)
 constexpr bool grav_has(int grav, int d, bool sph = false) {
   return (grav == GRAV_ANY && !(sph && d == 2)) || (grav == GRAV_Z && d == 2) || (grav == GRAV_R && d == 0);   // spherical builds: never along phi
@@ -77,6 +79,9 @@ constexpr bool grav_has(int grav, int d, bool sph = false) {
 struct Args {
   StepArgs s;
   int zc;            // planes per z chunk
+  int bcx_lo, bcx_hi; // boundary conditions of direction 0: the owners of the first / last two cells of a row also write the x-ghost
+                      // images of their cells (A0 for direction 0 folded into the update: the data is in registers, and x-ghost
+                      // columns are the expensive part of a separate fill -- one 64-byte DRAM burst per 16 useful bytes)
   // UNI instantiations only (bitwise-uniform Cartesian tables): constants of the three axes
   double uf[3];      // hw * idx   (slope pre-scale, = 1/2 up to rounding), times lim_scale of a build with a static limiter (1/2 for MC)
   double uhc[3];     // (dt/2) / delta_d
@@ -786,6 +791,11 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   const int k0 = blockIdx.z * a.zc, k1 = min(L.n[2], k0 + a.zc);
   const int i = i0 + ex, j = j0 + ey;                       // interior indices of this thread's column
   const bool st_ok = owner && i < L.n[0] && j < L.n[1];
+  // x-ghost images written by the boundary threads: only where the owner path has registers to spare -- the constant-geometry
+  // eight-row builds (rt_3d +1.9 %, cold_stream_3d +2.0 % whole step; the spherical builds lose 3-5 % in the kernel, the twelve-row
+  // build gains nothing: there the separate fill does it)
+  constexpr bool XG = writes_x_ghosts(UNI, TY);
+  const bool xedge = XG && st_ok && (i < NG || i >= L.n[0] - NG);
   const int cidx = (ey + 2) * PX + (ex + 2);                // offset of the own cell inside one field of a plane
   const int xs_own = ey * XP + ex + 1, xs_nbr = ey * XP + ex;
   const int ys_own = (ey + 1) * TX + ex, ys_nbr = ey * TX + ex;
@@ -1368,6 +1378,31 @@ step_tile2_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
         if (st_l) {
 #pragma unroll
           for (int v = 0; v < NV; ++v) outp[v * L.sv] = Unew[v];
+          if (XG && xedge) {   // x-ghost images of this cell (R16: both null-gradient layers copy the boundary cell; reflecting: mirror, -m_x)
+            const int n0 = L.n[0];
+            auto put = [&](int off, bool neg) {
+#pragma unroll
+              for (int v = 0; v < NV; ++v) outp[v * L.sv + off] = (v == 1 && neg) ? -Unew[v] : Unew[v];
+            };
+            if (i < NG) {                                  // one of the first two cells
+              if (a.bcx_hi == HX_BC_PERIODIC) put(n0, false);
+              if (a.bcx_lo == HX_BC_TRANSMISSIVE) {
+                if (i == 0) {
+                  put(-1, false);
+                  put(-2, false);
+                }
+              } else if (a.bcx_lo != HX_BC_PERIODIC) put(-1 - 2 * i, true);
+            }
+            if (i >= n0 - NG) {                            // one of the last two cells
+              if (a.bcx_lo == HX_BC_PERIODIC) put(-n0, false);
+              if (a.bcx_hi == HX_BC_TRANSMISSIVE) {
+                if (i == n0 - 1) {
+                  put(1, false);
+                  put(2, false);
+                }
+              } else if (a.bcx_hi != HX_BC_PERIODIC) put(2 * (n0 - 1 - i) + 1, true);
+            }
+          }
         }
 #pragma unroll
         for (int v = 0; v < 5; ++v) Ul[v] = Unew[v];

@@ -11,6 +11,8 @@ struct Plan {
   int ndim;          // 3: hx_step_tile2.cuh (march along z); 2: hx_step_tile2d.cuh (march along y)
   int zc;            // planes (rows in 2-D) per chunk of the march direction
   int ty;            // owner rows of a 3-D tile: 8, or 12 for the configuration tile_rows() names
+  int bcx_lo, bcx_hi; // boundary conditions of direction 0 (some 3-D builds write the x-ghost cells themselves)
+  bool xghost;       // the build launched last wrote the x-ghost cells of the interior rows (set by launch_cfg)
   dim3 grid;
   bool uni;          // bitwise-uniform Cartesian tables: geometry travels as kernel-parameter constants
   bool grav_z;       // uniform gravity along direction 2 only
@@ -47,6 +49,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a_in, int cur, cudaStream_
   const size_t smem = Smem<NV, TY>::total(plan.zc, SPH);
   cudaError_t e = set_smem_limit((const void*)kern, smem);
   if (e != cudaSuccess) return e;
+  plan.xghost = writes_x_ghosts(UNI, TY);
   plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? (TY == 12 ? "tile2_uni12" : "tile2_uni") : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
   kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();

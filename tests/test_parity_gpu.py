@@ -400,6 +400,29 @@ def test_uniform_grid_runtime_switch_builds(hx, oxlib, name, lim, riemann):
     assert max(l1) <= TOL_L1, (name, l1)
 
 
+@pytest.mark.parametrize("n0", [2, 4, 64])
+@pytest.mark.parametrize("bcx", [(0, 0), (1, 1), (2, 2), (2, 1), (1, 2)], ids=["periodic", "transmissive", "reflecting", "refl_trans", "trans_refl"])
+def test_x_ghosts_written_by_the_step_kernel(hx, oxlib, n0, bcx):
+    """The constant-geometry eight-row builds write the x-ghost images of their first / last two cells themselves (A0 for direction
+    0 folded into the update) and the fill that follows skips those columns: every x boundary type, down to n0 = 2 where a cell is
+    both a first and a last cell.  Four steps, so that steps 2-4 run on ghost cells the kernel wrote."""
+    ox = oxlib
+    spec, W = wl.smooth_periodic(3, [n0, 16, 8], seed=40 + n0, n_scalars=1, limiter=wl.LIM_MC)
+    spec = dict(spec)
+    spec["bc_lo"], spec["bc_hi"] = [bcx[0], 0, 2], [bcx[1], 0, 2]
+    W = W.copy()
+    W[0] += 0.5 * (W[2] > 0.0)
+    g, o = make_pair(hx, ox, spec, W)
+    for s in range(4):
+        dt = o.compute_dt(0.5)
+        assert abs(g.compute_dt(0.5) - dt) <= 1e-12 * dt, s
+        g.step(dt)
+        o.step(dt)
+    assert g.step_kernel == "tile2_uni"
+    rel = max_rel_per_field(g.get_state(), o.get_state(), 3)
+    assert max(rel) <= 4 * TOL_STEP, (n0, bcx, rel)
+
+
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times --------------------------------
 # (workload, expected step kernel, steps the GPU advances before the compared step: 0 = the initial state, 20 = a
 # late state in which the limiter and HLLC branches have switched on over the whole perturbed region)
