@@ -40,6 +40,7 @@ namespace {
 
 constexpr int NG = 2;       // ghost layers per face in active directions
 constexpr int NVMAX = 16;   // 2 + 3 + up to 11 passive scalars
+constexpr int NFMAX = NVMAX + 2;   // a face flux vector: the fields + the advective flux of e and the face velocity (monitoring, R29)
 
 inline bool is_reflecting(int bc) { return bc == OX_BC_REFLECTING || bc == OX_BC_WEDGE; }
 
@@ -888,7 +889,7 @@ int ox_step(ox_handle* h, double dt) {
           int a[3] = {i, j, k};
           a[d] -= 1;
           const size_t cl = h->cell(a[0], a[1], a[2]), cr = h->cell(i, j, k);
-          double UL[NVMAX], UR[NVMAX], Fl[NVMAX];
+          double UL[NVMAX], UR[NVMAX], Fl[NFMAX];
           for (int v = 0; v < nvar; ++v) {
             UL[v] = Up[d][(size_t)v * ncp + cl];
             UR[v] = Um[d][(size_t)v * ncp + cr];
@@ -905,7 +906,7 @@ int ox_step(ox_handle* h, double dt) {
     for (int j = 0; j < c.n[1]; ++j)
       for (int i = 0; i < c.n[0]; ++i) {
         const size_t ci = h->cell(i, j, k);
-        double Un[NVMAX], Fm[3][NVMAX], Fp[3][NVMAX], out[NVMAX];
+        double Un[NVMAX], Fm[3][NFMAX], Fp[3][NFMAX], out[NVMAX];
         for (int v = 0; v < nvar; ++v) Un[v] = U[(size_t)v * ncp + ci];
         for (int d = 0; d < ndim; ++d) {
           int b[3] = {i, j, k};
@@ -931,7 +932,7 @@ int ox_cell_update(ox_handle* h, int i, int j, int k, double dt, double* out) {
   const ox_config& c = h->c;
   if (i < 0 || i >= c.n[0] || j < 0 || j >= c.n[1] || k < 0 || k >= c.n[2]) return OX_ERR_INVALID_ARG;
   refresh_self_gravity(h);
-  double Un[NVMAX], Fm[3][NVMAX], Fp[3][NVMAX];
+  double Un[NVMAX], Fm[3][NFMAX], Fp[3][NFMAX];
   naive_get_U(h, i, j, k, Un);
   for (int d = 0; d < c.ndim; ++d) {
     int b[3] = {i, j, k};
