@@ -45,6 +45,7 @@ WORKLOADS = {
     "wedge_3d_sn": (lambda: wl.wedge_3d_sn((1024, 256, 256)), lambda: wl.wedge_3d_sn((96, 24, 24))),   # rad EOS + 5 scalars + point mass
     "wedge_3d_selfgrav": (lambda: wl.wedge_3d_selfgrav((1024, 256, 256)), lambda: wl.wedge_3d_selfgrav((192, 48, 48))),   # Eq. 4
     "wedge_3d_emon": (lambda: wl.wedge_3d_emon((1024, 256, 256)), lambda: wl.wedge_3d_emon((192, 48, 48))),   # SURVEY 8(f) rank 2 on the spherical wedge
+    "wedge_3d_sn_emon": (lambda: wl.wedge_3d_sn_emon((1024, 256, 256)), lambda: wl.wedge_3d_sn_emon((96, 24, 24))),   # rad EOS + 5 scalars + point mass + monitoring
     "cold_stream_3d": (lambda: wl.cold_stream_3d(256), lambda: wl.cold_stream_3d(64)),   # Eq. 10-12
     "kh_2d": (lambda: wl.kh_2d(1024), lambda: wl.kh_2d(512)),
     "sod_1d": (lambda: wl.sod_1d(1000), lambda: wl.sod_1d(1000)),

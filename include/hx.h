@@ -104,7 +104,7 @@ int hx_compute_dt(hx_handle* h, double cfl, double* dt_out);
 int hx_step(hx_handle* h, double dt);
 /* Number of stored fields, 2 + ndim + n_scalars. */
 int hx_nvar(const hx_handle* h);
-/* Name of the step kernel the last hx_step used ("generic", "tile2", "tile2_uni", "tile2_uni12", "tile2_rad", "tile2_emon", "tile2_emon_uni", "tile2d", "tile2d_uni"). */
+/* Name of the step kernel the last hx_step used ("generic", "tile2", "tile2_uni", "tile2_uni12", "tile2_rad", "tile2_rad_emon", "tile2_emon", "tile2_emon_uni", "tile2d", "tile2d_uni"). */
 const char* hx_step_kernel_name(const hx_handle* h);
 const char* hx_last_error(const hx_handle* h);
 const char* hx_version(void);

@@ -15,7 +15,7 @@ SOURCES = ["hx_host.cu", "hx_aux.cu", "hx_step_generic.cu", "hx_probe.cu", "hx_n
            "hx_step_tile2.cu", "hx_step_tile2_nv5.cu", "hx_step_tile2_nv6.cu", "hx_step_tile2_nv7.cu", "hx_step_tile2_nv9.cu", "hx_step_tile2_nv9_rad.cu", "hx_step_tile2d.cu",
            "hx_step_tile2_nv8.cu", "hx_step_tile2_nv10.cu", "hx_step_tile2_nv11.cu", "hx_step_tile2_nv5_rad.cu", "hx_step_tile2_nv6_rad.cu",
            "hx_step_tile2_nv7_rad.cu", "hx_step_tile2_nv8_rad.cu", "hx_step_tile2_nv10_rad.cu", "hx_step_tile2_nv11_rad.cu"] + \
-          ["hx_step_tile2_nv%d_emon.cu" % nv for nv in range(5, 12)]
+          ["hx_step_tile2_nv%d_emon.cu" % nv for nv in range(5, 12)] + ["hx_step_tile2_nv%d_rad_emon.cu" % nv for nv in range(5, 12)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -69,7 +69,6 @@ static bool nv_supported(int nv) { return nv >= 5 && nv <= 11; }
 int tile2_supported(const Layout& L, const Phys& P) {
   if (L.ndim == 2) return tile2d_supported(L, P);
   if (P.spherical && P.gravity == HX_GRAV_UNIFORM) return 0;   // a constant (r, theta, phi) acceleration vector: generic kernel (the spherical tile builds carry no phi gravity)
-  if (P.emon_eps > 0.0 && P.eos != HX_EOS_IDEAL) return 0;   // internal-energy monitoring (Eq. 10-12) with the gas + radiation EOS: generic kernel
   return L.ndim == 3 && nv_supported(L.nvar) && L.n[0] >= 2 && L.n[1] >= 2 && L.n[2] >= 2;
 }
 

@@ -50,7 +50,7 @@ static cudaError_t launch_cfg(Plan& plan, const Args& a_in, int cur, cudaStream_
   cudaError_t e = set_smem_limit((const void*)kern, smem);
   if (e != cudaSuccess) return e;
   plan.xghost = writes_x_ghosts(UNI, TY);
-  plan.name = EMON ? (UNI ? "tile2_emon_uni" : "tile2_emon") : (UNI ? (TY == 12 ? "tile2_uni12" : "tile2_uni") : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
+  plan.name = EMON ? (EOS != HX_EOS_IDEAL ? "tile2_rad_emon" : (UNI ? "tile2_emon_uni" : "tile2_emon")) : (UNI ? (TY == 12 ? "tile2_uni12" : "tile2_uni") : (EOS == HX_EOS_IDEAL ? "tile2" : "tile2_rad"));
   kern<<<plan.grid, (TY + 4) * 32, smem, st>>>(plan.tmap[cur], a);
   return cudaGetLastError();
 }

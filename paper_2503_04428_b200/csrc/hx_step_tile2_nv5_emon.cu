@@ -2,8 +2,10 @@
 #include "hx_step_tile2_launch.cuh"
 namespace hx {
 namespace t2 {
+cudaError_t launch_nv5_rad_emon(Plan& plan, const Args& a, int cur, cudaStream_t st);
 template <>
 cudaError_t launch_emon<5>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv5_rad_emon(plan, a, cur, st);   // own translation unit
   const Phys& P = a.s.P;
   // fully specialised: Cartesian, no gravity, MC + HLLC (cold_stream_3d)
   if (!P.spherical && P.gravity == HX_GRAV_NONE && P.limiter == HX_LIM_MC && P.riemann == HX_RIEMANN_HLLC) {

@@ -2,8 +2,10 @@
 #include "hx_step_tile2_launch.cuh"
 namespace hx {
 namespace t2 {
+cudaError_t launch_nv9_rad_emon(Plan& plan, const Args& a, int cur, cudaStream_t st);
 template <>
 cudaError_t launch_emon<9>(Plan& plan, const Args& a, int cur, cudaStream_t st) {
+  if (a.s.P.eos == HX_EOS_GAS_RADIATION) return launch_nv9_rad_emon(plan, a, cur, st);   // own translation unit
   const Phys& P = a.s.P;
   // fully specialised: spherical wedge, radial gravity, minmod + HLLC (wedge_3d_emon: the paper's use case, highly supersonic ejecta, L120-L126)
   if (P.spherical && plan.grav_r && P.limiter == HX_LIM_MINMOD && P.riemann == HX_RIEMANN_HLLC)

@@ -238,7 +238,7 @@ def wedge_3d_sn(n=(1024, 256, 256), seed=1005):
     return spec, W
 
 
-def wedge_3d_emon(n=(1024, 256, 256), seed=1007):
+def wedge_3d_emon(n=(1024, 256, 256), seed=1007, n_scalars=4):
     """SURVEY 8(f) rank 2 in the geometry the paper uses it for ("highly supersonic" supernova ejecta):
     the C5 wedge (same grid, density, pressure without the bomb, four composition shells, point-mass gravity) as a cold
     radial outflow u_r = 500 (Mach 800 at r = 1, 8000 at r = 100) with seeded velocity noise of 0.3 c_s in all three
@@ -246,7 +246,7 @@ def wedge_3d_emon(n=(1024, 256, 256), seed=1007):
     e / e_k = 6.8e-6 / r: alpha = 1 inside r ~ 7, the blended branch of Eq. 12 out to r ~ 68, alpha = 0 (internal energy
     from Eq. 10 alone) beyond.  (A homologous outflow u_r ~ r at this Mach number breaks the scheme in its first step
     with or without monitoring: the Hancock predictor forms its pressures from the total energy, R29.)"""
-    spec, W = wedge_3d(n, seed)
+    spec, W = wedge_3d(n, seed, n_scalars=n_scalars)
     nr, nt, nph = n
     spec = dict(spec, name="wedge_3d_emon", emon_eps=1e-6)
     spec["bc_lo"] = [BC_TRANSMISSIVE, BC_WEDGE, BC_WEDGE]
@@ -256,6 +256,15 @@ def wedge_3d_emon(n=(1024, 256, 256), seed=1007):
     W[1] = 500.0 + 0.3 * cs[None, None, :] * noise(seed + 1, (nph, nt, nr))
     W[2] = 0.3 * cs[None, None, :] * noise(seed + 2, (nph, nt, nr))
     W[3] = 0.3 * cs[None, None, :] * noise(seed + 3, (nph, nt, nr))
+    return spec, W
+
+
+def wedge_3d_sn_emon(n=(1024, 256, 256), seed=1007):
+    """Everything the paper's supernova runs switch on at once: the cold supersonic outflow of
+    wedge_3d_emon with five composition shells (nvar 10), the gas + radiation EOS (gas gamma 5/3, k_b/mu = 1, a_r = 30 as in
+    wedge_3d_rad: the same rho and P give P_r / P_g of 0.02-0.15), point-mass gravity and the monitoring of the internal energy."""
+    spec, W = wedge_3d_emon(n, seed, n_scalars=5)
+    spec = dict(spec, name="wedge_3d_sn_emon", gamma=5.0 / 3.0, eos=EOS_GAS_RADIATION, eos_R=1.0, eos_ar=30.0)
     return spec, W
 
 

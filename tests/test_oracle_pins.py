@@ -556,6 +556,12 @@ CASES_P11 = [
     ("c3d_emon", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 1),
     ("s3d_emon", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 1),
     ("c2d_hll_emon", 2, [7, 6], 0, [2, 0], [1, 0], 0, 2, 0, 0),
+    # both at once (the paper's supernova runs: gas + radiation EOS with the monitoring on)
+    ("s3d_rad_emon", 3, [6, 4, 5], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 2),
+    ("c3d_hll_rad_emon", 3, [6, 5, 4], 0, [0, 2, 1], [0, 2, 1], 1, 4, 0, 1),
+    # the maximum field count (16 stored fields; with the monitoring on a face flux vector carries 18 entries)
+    ("s3d_max_emon", 3, [6, 5, 4], 1, [2, 3, 0], [1, 3, 0], 2, 2, 0, 11),
+    ("c1d_max", 1, [12], 0, [1], [2], 1, 4, 1, 13),
 ]
 
 
@@ -579,9 +585,9 @@ def random_problem(ox, case, seed=0):
         kw.update(gravity=ox.GRAV_POINT_MASS, GM=0.8)
     elif grav == 3:
         kw.update(gravity=ox.GRAV_SELF, GM=0.8, G=0.6)
-    if name.endswith("_emon"):
+    if "_emon" in name:
         kw.update(emon_eps=5.0)
-    if name.endswith("_rad"):
+    if "_rad" in name:
         kw.update(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0)
     spec = wl._spec(name, ndim, n, faces, bc_lo, bc_hi, 1.4, lim, **kw)
     shape = tuple((n + [1, 1])[:3][::-1])

@@ -61,6 +61,7 @@ REDUCED = {
     "wedge_3d_selfgrav": lambda: wl.wedge_3d_selfgrav((72, 18, 20)),   # SURVEY 8(f) rank 4 (self-gravity, Eq. 4)
     "cold_stream_3d": lambda: wl.cold_stream_3d((40, 24, 20)),           # SURVEY 8(f) rank 2 (internal-energy monitoring, Eq. 10-12)
     "wedge_3d_emon": lambda: wl.wedge_3d_emon((104, 22, 26)),            # ... in the geometry the paper uses it for: supersonic ejecta in the spherical wedge
+    "wedge_3d_sn_emon": lambda: wl.wedge_3d_sn_emon((104, 22, 26)),      # ... with the gas + radiation EOS and five scalars on top
 }
 
 
@@ -183,6 +184,8 @@ FIELD_CASES = [
     ("s3d_ns0_emon", 3, [36, 10, 7], 1, [2, 3, 0], [1, 3, 0], 2, 1, 1, 0),
     ("s3d_ns4_hll_emon", 3, [36, 10, 7], 1, [2, 3, 3], [1, 3, 3], 2, 2, 0, 4),
     ("c3d_ns6_emon", 3, [37, 11, 6], 0, [2, 1, 2], [1, 2, 2], 0, 1, 1, 6),
+    ("s3d_ns5_rad_emon", 3, [36, 10, 7], 1, [2, 3, 3], [1, 3, 3], 2, 1, 1, 5),
+    ("c3d_ns1_rad_emon", 3, [37, 11, 6], 0, [0, 2, 1], [0, 2, 1], 1, 4, 0, 1),
     ("c2d_ns0", 2, [300, 9], 0, [2, 0], [1, 0], 1, 2, 1, 0),
     ("c2d_ns2", 2, [261, 12], 0, [0, 1], [0, 2], 1, 4, 1, 2),
     ("c2d_ns4_hll", 2, [70, 40], 0, [1, 2], [2, 1], 0, 1, 0, 4),
@@ -200,10 +203,37 @@ def test_every_field_count_on_the_tile_kernels(hx, oxlib, case):
         assert abs(0.5 * g.compute_dt(0.5) - dt) <= 1e-13 * dt
         g.step(dt)
         o.step(dt)
-    want = "tile2d" if spec["ndim"] == 2 else ("tile2_rad" if spec["eos"] else ("tile2_emon" if spec["emon_eps"] > 0 else "tile2"))
+    want = "tile2d" if spec["ndim"] == 2 else {(0, False): "tile2", (1, False): "tile2_rad", (0, True): "tile2_emon",
+                                               (1, True): "tile2_rad_emon"}[(spec["eos"], spec["emon_eps"] > 0)]
     assert g.step_kernel == want, (case[0], g.step_kernel)
     rel = max_rel_per_field(g.get_state(), o.get_state(), spec["ndim"])
     assert max(rel) <= 3 * TOL_STEP, (case[0], rel)
+
+
+MAX_FIELD_CASES = [   # HX_MAX_NVAR = 16 stored fields in 1-D, 2-D, 3-D: beyond the tile kernels' field counts, on the generic kernel
+    ("c1d_max", 1, [40], 0, [1], [2], 1, 4, 1, 13),
+    ("c2d_max", 2, [33, 9], 0, [0, 2], [0, 1], 1, 1, 1, 12),
+    ("s3d_max", 3, [34, 9, 6], 1, [2, 3, 0], [1, 3, 0], 2, 2, 0, 11),
+    ("c3d_max_rad", 3, [33, 9, 6], 0, [0, 2, 1], [0, 2, 1], 1, 4, 1, 11),
+]
+
+
+@pytest.mark.parametrize("case", MAX_FIELD_CASES, ids=[c[0] for c in MAX_FIELD_CASES])
+def test_maximum_field_count(hx, oxlib, case):
+    ox = oxlib
+    spec, W = random_problem(ox, case)
+    assert spec["nvar"] == 16
+    g, o = make_pair(hx, ox, spec, W, "auto")
+    for _ in range(3):
+        dt = 0.5 * o.compute_dt(0.5)
+        assert abs(0.5 * g.compute_dt(0.5) - dt) <= 1e-13 * dt
+        g.step(dt)
+        o.step(dt)
+    assert g.step_kernel == "generic"
+    rel = max_rel_per_field(g.get_state(), o.get_state(), spec["ndim"])
+    assert max(rel) <= 3 * TOL_STEP, (case[0], rel)
+    with pytest.raises(hx.HxError):                 # one field more is rejected at hx_create
+        hx.Hydro(dict(spec, n_scalars=spec["n_scalars"] + 1, nvar=17))
 
 
 @pytest.mark.parametrize("lim", [0, 1, 2, 3, 4])
@@ -439,6 +469,7 @@ FULL = {
     "cold_stream_3d_late": (lambda: wl.cold_stream_3d(256), "tile2_emon_uni", 20),
     "wedge_3d_emon": (lambda: wl.wedge_3d_emon((1024, 256, 256)), "tile2_emon", 0),
     "wedge_3d_emon_late": (lambda: wl.wedge_3d_emon((1024, 256, 256)), "tile2_emon", 20),
+    "wedge_3d_sn_emon": (lambda: wl.wedge_3d_sn_emon((1024, 256, 256)), "tile2_rad_emon", 0),
 }
 
 
