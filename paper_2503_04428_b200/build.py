@@ -33,19 +33,28 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
         return lib
     os.makedirs(objdir, exist_ok=True)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    objs = []
-    procs = []
-    for src in SOURCES:
-        obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
-        procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
-        objs.append(obj)
-    for src, p in procs:
+    # one nvcc per translation unit, at most `jobs` at a time (HX_BUILD_JOBS, default: the cores of this box): 44 compilers at once
+    # need tens of GB of memory; the heaviest units (gas + radiation EOS builds) go first so that they do not end up alone at the tail
+    jobs = max(1, int(os.environ.get("HX_BUILD_JOBS", "0")) or (os.cpu_count() or 4))
+    order = sorted(SOURCES, key=lambda f: (0 if "_rad" in f else 1 if "tile2" in f else 2))
+    objs = [os.path.join(objdir, src.replace(".cu", ".o")) for src in SOURCES]
+    pending, running, failed = list(order), [], None
+    while (pending or running) and failed is None:
+        while pending and len(running) < jobs:
+            src = pending.pop(0)
+            obj = os.path.join(objdir, src.replace(".cu", ".o"))
+            cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+            running.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+        src, p = running.pop(0)                 # wait for the oldest one (they finish roughly in order)
         out, _ = p.communicate()
         if verbose or p.returncode != 0:
             sys.stderr.write(out)
         if p.returncode != 0:
-            raise RuntimeError(f"nvcc failed on {src}")
+            failed = src
+    for _, p in running:
+        p.kill()
+    if failed is not None:
+        raise RuntimeError(f"nvcc failed on {failed}")
     cmd = [nvcc, "-shared", "-o", lib] + objs + ["-lcudart", "-lcuda"]
     subprocess.run(cmd, check=True)
     return lib
