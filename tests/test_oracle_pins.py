@@ -997,13 +997,17 @@ def test_p14_monitoring_keeps_a_cold_supersonic_stream_cold(oxlib):
     assert drift[1e-6] <= 1e-4 * drift[0.0] or drift[1e-6] <= 1e-12, drift
 
 
-def test_p14_second_energy_equation_compression_work(oxlib):
-    """Eq. 10 with uniform rho, e, P and u = a x: de/dt = -(e + P) a.  eps huge puts every cell on the alpha = 0
-    branch; one small step changes e by -(e + P) a dt in the interior (first order in dt and dx)."""
+@pytest.mark.parametrize("eos", ["ideal", "gas_radiation"])
+def test_p14_second_energy_equation_compression_work(oxlib, eos):
+    """Eq. 10 with uniform rho, e, P and u = a x: de/dt = -(e + P) a, whatever the equation of state (with the gas + radiation
+    EOS of Eq. 6, P_r / P_g ~ 1 here, e is no longer P / (gamma - 1): the pin checks that Eq. 10 takes P and e from the EOS).
+    eps huge puts every cell on the alpha = 0 branch; one small step changes e by -(e + P) a dt in the interior (first order in
+    dt and dx)."""
     ox = oxlib
     n, a = 64, 0.05
     fx = wl.uniform_faces(0.0, 1.0, n)
-    spec = wl._spec("emon1d", 1, [n], [fx], [wl.BC_TRANSMISSIVE], [wl.BC_TRANSMISSIVE], 1.4, wl.LIM_MC, emon_eps=1e30)
+    kw = dict(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0) if eos == "gas_radiation" else {}
+    spec = wl._spec("emon1d", 1, [n], [fx], [wl.BC_TRANSMISSIVE], [wl.BC_TRANSMISSIVE], 1.4, wl.LIM_MC, emon_eps=1e30, **kw)
     x = 0.5 * (fx[1:] + fx[:-1])
     W = np.empty((3, 1, 1, n))
     W[0], W[1, 0, 0], W[2] = 1.0, a * (x - 0.5), 2.0
