@@ -2,16 +2,17 @@
 //
 // The 2-D counterpart of hx_step_tile2.cuh (config 2 of BASELINE.json, the Kelvin-Helmholtz run of PAPER.md
 // Sect. 4.1; "1D, 2D, or 3D", L149).  Same design, one dimension down:
-//   * a CTA owns a strip of NW x 32 cells in x (warp <-> 32-cell segment, lane <-> cell) and marches along y over a
-//     chunk of rows; a row (strip + 2 ghost cells on each side, all fields) arrives by ONE TMA bulk-tensor copy into a
-//     3-deep ring signalled by mbarriers; cons -> prim runs in place;
+//   * a CTA owns a strip of NW x 32 = 352 cells in x (warp <-> 32-cell segment, lane <-> cell) and marches along y over a
+//     chunk of rows; a row (strip + 2 ghost cells on each side, all fields) arrives by TWO TMA bulk-tensor copies (a box is at
+//     most 256 elements wide) into a 3-deep ring signalled by mbarriers; cons -> prim runs in place;
 //   * y is the march direction: the y slopes, the predicted y+ state of the previous row and the partially updated
 //     cell of the previous row stay in registers;
 //   * x neighbours exchange through shared memory: a cell writes the predicted state of its x+ face into its own
 //     slot, the neighbour across that face solves the Riemann problem ONCE and writes the flux back into the same
 //     slot; the slots are double buffered by row parity so that ONE CTA-wide barrier per row suffices;
-//   * the two cells of the one-cell ring left and right of the strip are handled by two lanes of one extra warp (its
-//     warpgroup gives registers back with setmaxnreg, the two owner warpgroups take them);
+//   * the two cells of the one-cell ring left and right of the strip are handled by two lanes of one extra warp; with eleven
+//     owner warps it completes the third warpgroup, so that every scheduler holds three warps (a ring warp in a warpgroup of its
+//     own, rebalanced with setmaxnreg as in 3-D, leaves one scheduler with one warp more than the others: measured slower);
 //   * the CFL rate of a cell is folded in one row after it was written (A7), reduced by warp shuffles, one atomicMax
 //     per CTA.
 // Pointwise arithmetic as in the 3-D kernel (reciprocal / square root = MUFU seed + cubic correction, limiters on
@@ -41,7 +42,16 @@ using t2::smem_u32;
 using t2::sqrt3;
 using t2::sqrt3_n;
 
-constexpr int NW = 8;                 // owner warps = 32-cell segments of the strip (two warpgroups)
+#ifndef HX_T2D_NW
+#define HX_T2D_NW 11   // measured on kh_2d 1024^2 (kernel ms): 8 owners + ring warpgroup 0.0595 (scheduler 0 carries three warps, the others
+                       // two: the barrier waits for it), 7 + 1 0.0588 (balanced, but 1024 = 4.6 strips), 11 + 1 0.0528 (three warps per scheduler)
+#endif
+constexpr int NW = HX_T2D_NW;         // owner warps = 32-cell segments of the strip
+// NW a multiple of 4: the ring warp gets a warpgroup of its own (three idle warps) and gives registers back (setmaxnreg).
+// Otherwise the ring warp shares the last warpgroup with owners (NW + 1 a multiple of 4: every scheduler holds the same number of
+// warps) and all warps keep the launch allocation.
+constexpr bool REBAL = NW % 4 == 0;
+static_assert(REBAL || (NW + 1) % 4 == 0, "NW or NW + 1 must be a multiple of 4");
 constexpr int TXS = NW * 32;          // owner cells per strip row
 constexpr int PXS = TXS + 4;          // staged row: strip + 2 ghost cells on each side
 constexpr int HXS = PXS / 2;          // a TMA box is at most 256 elements wide: a row arrives as two halves of 130 cells (1040 B each),
@@ -50,14 +60,14 @@ constexpr int HXS = PXS / 2;          // a TMA box is at most 256 elements wide:
 constexpr int half_stride(int nv) { return (nv * HXS * 8 + 127) / 128 * 128 / 8; }
 // offset of cell c (0 .. PXS-1) of field 0 inside a staged row of nv fields; the field stride is HXS
 __device__ __forceinline__ int row_off(int c, int nv) { return c < HXS ? c : half_stride(nv) + (c - HXS); }
-constexpr int NTHREADS = (NW + 4) * 32;
-constexpr int REGS_LAUNCH = (65536 / NTHREADS) / 8 * 8;   // 168
+constexpr int NTHREADS = (REBAL ? NW + 4 : NW + 1) * 32;
+constexpr int REGS_LAUNCH = (65536 / NTHREADS) / 8 * 8;   // 168 with twelve warps
 #ifndef HX_T2D_REGS_RING
 #define HX_T2D_REGS_RING 136   // measured on kh_2d 1024^2: 104 (spills in the ring path) 0.0705 ms, 120 0.0650, 136 0.0586, 152 0.0600, 168 0.0582
 #endif
 constexpr int REGS_RING = HX_T2D_REGS_RING;
-constexpr int REGS_OWNER = (REGS_LAUNCH * (NW + 4) - REGS_RING * 4) / NW / 8 * 8;   // 200
-static_assert(REGS_OWNER * NW + REGS_RING * 4 <= REGS_LAUNCH * (NW + 4), "setmaxnreg budgets exceed the launch allocation");
+constexpr int REGS_OWNER = REBAL ? (REGS_LAUNCH * (NW + 4) - REGS_RING * 4) / NW / 8 * 8 : REGS_LAUNCH;   // 184
+static_assert(!REBAL || REGS_OWNER * NW + REGS_RING * 4 <= REGS_LAUNCH * (NW + 4), "setmaxnreg budgets exceed the launch allocation");
 
 enum { GRAV_OFF = 0, GRAV_ANY = 1 };
 
@@ -397,8 +407,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) step_tile2d_kernel(const __grid_c
     }
   }
   // register rebalancing, one setmaxnreg per warpgroup: the ring warpgroup gives registers back, the owners take them
-  if (owner) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_OWNER));
-  else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_RING));
+  if (REBAL) {
+    if (owner) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_OWNER));
+    else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_RING));
+  }
   if (wid > NW) {             // the rest of the ring warpgroup was only needed for setmaxnreg: wait in the final reduction
     block_rate_max(0.0, s.rate_bits);
     return;

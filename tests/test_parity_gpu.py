@@ -381,6 +381,20 @@ def test_tile_edges(hx, oxlib, n):
     assert max(max_rel_per_field(g.get_state(), o.get_state(), 3)) <= 2 * TOL_STEP, n
 
 
+@pytest.mark.parametrize("n", [(352, 9), (353, 10), (705, 6), (32, 5), (2, 2)])
+def test_strip_edges_2d(hx, oxlib, n):
+    """2-D grids of exactly one strip of the tile2d kernel (11 x 32 cells), one cell more, two strips and a cell, and tiny ones."""
+    ox = oxlib
+    spec, W = wl.smooth_periodic(2, list(n), seed=n[0], n_scalars=1, limiter=wl.LIM_MC)
+    g, o = make_pair(hx, ox, spec, W, "auto")
+    for _ in range(3):
+        dt = o.compute_dt(0.5)
+        g.step(dt)
+        o.step(dt)
+    assert g.step_kernel.startswith("tile2d")
+    assert max(max_rel_per_field(g.get_state(), o.get_state(), 2)) <= 2 * TOL_STEP, n
+
+
 UNIFORM = {   # 2^k cells on dyadic extents: bitwise-uniform tables -> the constant-geometry instantiations
     "sedov_3d": lambda: wl.sedov_3d((64, 32, 32)),
     "rt_3d": lambda: wl.rt_3d((32, 64, 64)),
