@@ -33,7 +33,7 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
         return lib
     os.makedirs(objdir, exist_ok=True)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    # one nvcc per translation unit, at most `jobs` at a time (HX_BUILD_JOBS, default: the cores of this box): 44 compilers at once
+    # one nvcc per translation unit, at most `jobs` at a time (HX_BUILD_JOBS, default: the cores of this box): 35 compilers at once
     # need tens of GB of memory; the heaviest units (gas + radiation EOS builds) go first so that they do not end up alone at the tail
     jobs = max(1, int(os.environ.get("HX_BUILD_JOBS", "0")) or (os.cpu_count() or 4))
     order = sorted(SOURCES, key=lambda f: (0 if "_rad" in f else 1 if "tile2" in f else 2))
