@@ -467,6 +467,67 @@ def test_x_ghosts_written_by_the_step_kernel(hx, oxlib, n0, bcx):
     assert max(rel) <= 4 * TOL_STEP, (n0, bcx, rel)
 
 
+def _random_case(seed):
+    """A seeded random 3-D configuration: (spec, W).  Even seeds: non-uniform grids through random_problem (Cartesian or spherical);
+    odd seeds: bitwise-uniform Cartesian grids (2^k cells on [0, 1]) so that the constant-geometry builds and their x-ghost writes
+    are drawn too."""
+    rng = np.random.default_rng(9000 + seed)
+    lim, riem, ns = int(rng.integers(0, 5)), int(rng.integers(0, 2)), int(rng.integers(0, 7))
+    flags = ["", "_rad", "_emon", "_rad_emon"][int(rng.integers(0, 4))]
+
+    def bc_pair(allow_periodic=True):
+        k = int(rng.integers(0 if allow_periodic else 1, 4))
+        if k == 0:
+            return 0, 0
+        return int(rng.integers(1, 3)), int(rng.integers(1, 3))
+    if seed % 2 == 0:
+        coords = int(rng.integers(0, 2))
+        n = [int(rng.integers(2, 70)), int(rng.integers(2, 20)), int(rng.integers(2, 12))]
+        b0, b1, b2 = bc_pair(allow_periodic=(coords == 0)), bc_pair(), bc_pair()
+        grav = int(rng.integers(0, 2)) if coords == 0 else int(rng.integers(2, 4)) if rng.integers(0, 2) else 0
+        case = (f"rnd{seed}{flags}", 3, n, coords, [b0[0], b1[0], b2[0]], [b0[1], b1[1], b2[1]], grav, lim, riem, ns)
+        return case, None
+    n = [int(2 ** rng.integers(1, 7)), int(2 ** rng.integers(1, 5)), int(2 ** rng.integers(1, 4))]
+    b0, b1, b2 = bc_pair(), bc_pair(), bc_pair()
+    spec, W = wl.smooth_periodic(3, n, seed=seed, n_scalars=ns, limiter=lim, riemann=riem)
+    spec = dict(spec, name=f"rnd{seed}{flags}")
+    spec["bc_lo"], spec["bc_hi"] = [b0[0], b1[0], b2[0]], [b0[1], b1[1], b2[1]]
+    if rng.integers(0, 2):
+        spec.update(gravity=wl.GRAV_UNIFORM, g=[0.0, 0.0, -0.4] if rng.integers(0, 2) else [0.3, -0.2, -0.5])
+    if "_rad" in flags:
+        spec.update(eos=wl.EOS_GAS_RADIATION, eos_R=1.0, eos_ar=2.0)
+    if "_emon" in flags:
+        spec.update(emon_eps=5.0)
+    W = W.copy()
+    W[0] += 0.6 * (W[1] > 0.05)
+    return None, (spec, W)
+
+
+@pytest.mark.parametrize("seed", range(32))
+def test_random_configurations_tile_generic_oracle(hx, oxlib, seed):
+    """Seeded random 3-D configurations on the fused tile kernel, on the generic kernel and in the oracle: three steps, all three agree."""
+    ox = oxlib
+    case, prob = _random_case(seed)
+    spec, W = random_problem(ox, case) if case is not None else prob
+    gt, o = make_pair(hx, ox, spec, W, "auto")
+    gg = hx.Hydro(spec)
+    gg.set_option(hx.OPT_KERNEL, hx.KERNEL_GENERIC)
+    gg.set_state(np.ascontiguousarray(W), hx.PRIMITIVE)
+    for _ in range(3):
+        dt = 0.5 * o.compute_dt(0.5)
+        assert abs(0.5 * gt.compute_dt(0.5) - dt) <= 1e-12 * dt and abs(0.5 * gg.compute_dt(0.5) - dt) <= 1e-12 * dt
+        gt.step(dt)
+        gg.step(dt)
+        o.step(dt)
+    Uo = o.get_state()
+    supported = not (spec["coords"] == 1 and spec["gravity"] == wl.GRAV_UNIFORM)
+    assert gt.step_kernel.startswith("tile2") == supported, (spec["name"], gt.step_kernel)
+    assert gg.step_kernel == "generic"
+    for g in (gt, gg):
+        rel = max_rel_per_field(g.get_state(), Uo, 3)
+        assert max(rel) <= 3 * TOL_STEP, (seed, spec["name"], g.step_kernel, rel)
+
+
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times --------------------------------
 # (workload, expected step kernel, steps the GPU advances before the compared step: 0 = the initial state, 20 = a
 # late state in which the limiter and HLLC branches have switched on over the whole perturbed region)
